@@ -1,0 +1,121 @@
+/*
+ * tri_attn.h -- C ABI of libtri_attn.so: fused forward / backward of AF3-style triangle attention
+ * with pair bias ("EvoAttention"; memory-efficient kernel "EvoFlash-3D") for NVIDIA B200 (sm_100a).
+ *
+ * What is computed (PAPER.md = /root/reference/PAPER.md of arxiv 2506.20686, cited P:L<line>):
+ *   forward   S = scale*Q K^T + Bias_bcast + M(mask);  P = softmax_k(S);  A = P V;  O = sigmoid(G) (.) A
+ *             Table I, Sec. IV-A, Listing 1 P:L153-185 (`fused_attn_fwd`).
+ *             scale = 1/sqrt(d), the sigmoid gate G and the additive -inf mask are fixed by the task
+ *             statement (BASELINE.json north_star), not by the paper (readings A1/A3/A4).
+ *   backward  dV = P^T dA, dP = dA V^T, dS = P (.) (dP - rowsum(dO (.) O)), dK = scale dS^T Q,
+ *             dQ = scale dS K, dBias = sum over the broadcast axis of dS, dA = dO (.) sigmoid(G),
+ *             dG = dO (.) O (.) (1 - sigmoid(G)).   Table I, Listing 2
+ *             (`fused_attn_bwd`: preprocess D, stage 1 dK/dV, stage 2 dQ/dBias).  The paper's
+ *             atomic_add of dS tiles is replaced by a deterministic two-level reduction.
+ *   The O(N^3) attention map [B,N,H,N,N] is never written to device memory.
+ *
+ * Tensor layouts (row-major, contiguous; "a" = first pair axis, "c" = second pair axis):
+ *   Q,K,V,G,O,dO,dQ,dK,dV,dG : [B, N, H, N, d]   element (b,a,h,c,:)      dtype = `dtype`
+ *   bias                     : [B, H, N, N]                               dtype = `dtype`
+ *   dBias                    : [B, H, N, N]                               float32 always
+ *   mask                     : [B, N, N] unsigned char keep flags (non-zero = visible), or NULL
+ *   LSE                      : [B, N, H, N] float32, natural-log units, element (b,a,h,c)
+ *
+ * Variants:
+ *   TRI_STARTING  row i = a, query j = c, key k = c':
+ *       S[b,i,h,j,k] = scale <Q[b,i,h,j,:],K[b,i,h,k,:]> + bias[b,h,j,k] + M(mask[b,i,k])
+ *       O[b,i,h,j,:] = sigmoid(G[b,i,h,j,:]) (.) sum_k P V[b,i,h,k,:];  dBias[b,h,j,k] = sum_i dS
+ *   TRI_ENDING    (= T . starting . T, T = swap of the two N axes of every argument)
+ *       S[b,i,h,j,k] = scale <Q[b,i,h,j,:],K[b,k,h,j,:]> + bias[b,h,k,i] + M(mask[b,k,j])
+ *       O[b,i,h,j,:] = sigmoid(G[b,i,h,j,:]) (.) sum_k P V[b,k,h,j,:];  dBias[b,h,k,i] = sum_j dS
+ *   A query whose keys are all masked gives O = 0, LSE = -inf and contributes zero gradients.
+ *
+ * Ownership and behaviour:
+ *   - Every tensor pointer of tri_attn_fwd / tri_attn_bwd is a caller-owned DEVICE pointer, 16-byte
+ *     aligned.  The library never allocates or frees device memory and never synchronises the
+ *     device: all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  Scratch space comes from `workspace` (device, 256-byte aligned, at
+ *     least *_workspace_bytes() bytes, contents undefined on entry and exit).  workspace_bytes is
+ *     O(B*H*N^2); nothing of size B*H*N^3 exists anywhere.
+ *   - Outputs must not alias inputs or each other; outputs are overwritten (dBias is NOT
+ *     accumulated into).  Results are bitwise reproducible run to run (no floating-point atomics).
+ *   - tri_attn_step_host takes HOST pointers (pinned memory recommended) for every tensor plus a
+ *     caller-owned DEVICE arena; it copies inputs in, runs forward + backward, copies results out,
+ *     all on `cuda_stream`, and does not synchronise.
+ *   - Errors: a tri_status is returned, nothing is thrown or aborted across the ABI.  Argument
+ *     errors are detected before any launch.  Launch failures map to TRI_ERR_CUDA.
+ *   - Supported: d in {16, 32, 64}, any N >= 1, dtype f32 or bf16.  bf16 with d == 32 and
+ *     N % 128 == 0 runs on the tcgen05/TMA tensor-core kernels; every other combination runs on
+ *     the fp32 CUDA-core kernels (fp32 needs them: the 1e-4 bound excludes TF32, reading A14).
+ *     Anything else returns TRI_ERR_UNSUPPORTED.  There is no CPU path.
+ */
+#ifndef TRI_ATTN_H_
+#define TRI_ATTN_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define TRI_API __attribute__((visibility("default")))
+#else
+#define TRI_API
+#endif
+
+typedef enum {
+    TRI_OK = 0,
+    TRI_ERR_INVALID_ARG = 1, /* NULL / misaligned pointer, non-positive size, bad enum            */
+    TRI_ERR_UNSUPPORTED = 2, /* shape or dtype outside the supported set                           */
+    TRI_ERR_WORKSPACE = 3,   /* workspace NULL / misaligned / smaller than *_workspace_bytes()      */
+    TRI_ERR_CUDA = 4         /* a CUDA runtime / driver call or a kernel launch failed             */
+} tri_status;
+
+typedef enum { TRI_F32 = 0, TRI_BF16 = 1 } tri_dtype;
+typedef enum { TRI_STARTING = 0, TRI_ENDING = 1 } tri_variant;
+
+/* Bytes of device scratch tri_attn_fwd / tri_attn_bwd need for this problem (0 on bad arguments). */
+TRI_API size_t tri_attn_fwd_workspace_bytes(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);
+TRI_API size_t tri_attn_bwd_workspace_bytes(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);
+
+/* Forward (Listing 1 P:L153-185 + gate + mask).  Inputs Q,K,V,G,bias,mask; outputs O, LSE. */
+TRI_API tri_status tri_attn_fwd(const void* Q, const void* K, const void* V, const void* G,
+                        const void* bias, const unsigned char* mask /* NULL = no mask */,
+                        void* O, float* LSE,
+                        int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Backward (Listing 2 P:L434-494 + gate).  O and LSE are the forward's outputs.
+ * Outputs dQ,dK,dV,dG (dtype) and dBias (float32). */
+TRI_API tri_status tri_attn_bwd(const void* dO,
+                        const void* Q, const void* K, const void* V, const void* G,
+                        const void* bias, const unsigned char* mask,
+                        const void* O, const float* LSE,
+                        void* dQ, void* dK, void* dV, void* dG, float* dBias,
+                        int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* End-to-end step on HOST buffers: H2D(Q,K,V,G,bias,mask,dO) -> fwd -> bwd -> D2H(O,LSE,dQ,dK,dV,
+ * dG,dBias).  `arena` is a caller-owned device buffer of tri_attn_step_host_arena_bytes() bytes. */
+TRI_API size_t tri_attn_step_host_arena_bytes(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);
+TRI_API tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, const void* hG,
+                              const void* hbias, const unsigned char* hmask, const void* hdO,
+                              void* hO, float* hLSE,
+                              void* hdQ, void* hdK, void* hdV, void* hdG, float* hdBias,
+                              int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
+                              void* arena, size_t arena_bytes, void* cuda_stream);
+
+/* Number of kernel launches this library has enqueued since it was loaded (for bench accounting). */
+TRI_API unsigned long long tri_attn_launch_count(void);
+
+/* Static description of a status code. */
+TRI_API const char* tri_status_string(tri_status s);
+
+/* Last CUDA error text recorded by a TRI_ERR_CUDA return on this thread ("" if none). */
+TRI_API const char* tri_attn_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRI_ATTN_H_ */

@@ -1,0 +1,89 @@
+// Internal declarations shared by the translation units of libtri_attn.so (not part of the ABI).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "tri_attn.h"
+
+namespace tri {
+
+// One problem instance.  Index conventions (include/tri_attn.h): a "slice" is one (b, r, h) where r
+// runs over the broadcast axis of the variant (i for starting, j for ending); inside a slice,
+// queries q and keys k run over the other pair axis.
+struct Problem {
+    int B, N, H, d;
+    int variant;  // tri_variant
+    // element strides of the [B,N,H,N,d] tensors
+    long long sB;      // N*H*N*d
+    long long sH;      // N*d
+    long long sSlice;  // starting: H*N*d (axis a)   ending: d (axis c)
+    long long sPos;    // starting: d     (axis c)   ending: H*N*d (axis a)
+    // bias[b,h,.,.] : element (q,k) at q*bQ + k*bK
+    int bQ, bK;
+    // mask[b,.,.]   : element (r,k) at r*mR + k*mK
+    int mR, mK;
+    // LSE / D [B,N,H,N]: element (r,q) at r*lR + q*lQ (+ b*N*H*N + h*N)
+    long long lR, lQ;
+};
+
+inline Problem make_problem(int B, int N, int H, int d, int variant) {
+    Problem p;
+    p.B = B; p.N = N; p.H = H; p.d = d; p.variant = variant;
+    p.sB = (long long)N * H * N * d;
+    p.sH = (long long)N * d;
+    if (variant == TRI_STARTING) {
+        p.sSlice = (long long)H * N * d; p.sPos = d;
+        p.bQ = N; p.bK = 1;
+        p.mR = N; p.mK = 1;
+        p.lR = (long long)H * N; p.lQ = 1;
+    } else {
+        p.sSlice = d; p.sPos = (long long)H * N * d;
+        p.bQ = 1; p.bK = N;
+        p.mR = 1; p.mK = N;
+        p.lR = 1; p.lQ = (long long)H * N;
+    }
+    return p;
+}
+
+// launch accounting + error capture (tri_attn_api.cu)
+void count_launch(int n = 1);
+tri_status cuda_fail(cudaError_t e, const char* where);
+#define TRI_CUDA_CHECK(expr)                                   \
+    do {                                                       \
+        cudaError_t _e = (expr);                               \
+        if (_e != cudaSuccess) return ::tri::cuda_fail(_e, #expr); \
+    } while (0)
+#define TRI_LAUNCH_CHECK(where)                                \
+    do {                                                       \
+        ::tri::count_launch();                                 \
+        cudaError_t _e = cudaGetLastError();                   \
+        if (_e != cudaSuccess) return ::tri::cuda_fail(_e, where); \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- fp32 CUDA-core path (simt_kernels.cu) -------------------------------------------------
+size_t simt_fwd_workspace(const Problem& p);
+size_t simt_bwd_workspace(const Problem& p);
+tri_status simt_fwd(const Problem& p, tri_dtype dt, const void* Q, const void* K, const void* V,
+                    const void* G, const void* bias, const unsigned char* mask, void* O, float* LSE,
+                    void* ws, cudaStream_t st);
+tri_status simt_bwd(const Problem& p, tri_dtype dt, const void* dO, const void* Q, const void* K,
+                    const void* V, const void* G, const void* bias, const unsigned char* mask,
+                    const void* O, const float* LSE, void* dQ, void* dK, void* dV, void* dG,
+                    float* dBias, void* ws, cudaStream_t st);
+
+// ---- bf16 tcgen05 / TMA path (sm100_fwd.cu, sm100_bwd.cu) ------------------------------------
+bool sm100_supported(const Problem& p, tri_dtype dt);
+size_t sm100_fwd_workspace(const Problem& p);
+size_t sm100_bwd_workspace(const Problem& p);
+tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void* V, const void* G,
+                     const void* bias, const unsigned char* mask, void* O, float* LSE, void* ws,
+                     cudaStream_t st);
+tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void* K, const void* V,
+                     const void* G, const void* bias, const unsigned char* mask, const void* O,
+                     const float* LSE, void* dQ, void* dK, void* dV, void* dG, float* dBias,
+                     void* ws, cudaStream_t st);
+
+}  // namespace tri
