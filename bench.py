@@ -1,0 +1,367 @@
+"""bench.py -- triangle-attention fwd+bwd TFLOP/s on synthetic AF3-crop pair tensors (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path: tri_attn_fwd followed by
+tri_attn_bwd through the C-ABI on one batch of synthetic input.  Default workload = BASELINE.json
+configs[3] ("cfg4": B=2, N=768, H=4, d=32, bf16, starting node, ragged key mask 700/768), the N=768
+configuration the metric is quoted on; it fits one GPU.  Model FLOP = 14*B*H*N^3*d (fwd 2 + bwd 5
+matmuls of 2*N^2*d each per (b,row,h)).
+
+Prints ONE JSON line (rank 0).  `value` = model TFLOP/s with inputs resident in HBM; `e2e` = the same
+metric through tri_attn_step_host with pinned HOST buffers (H2D + D2H inside the timed region);
+`roofline` = dominant kernel's model FLOP / its CUDA-event duration against the measured bf16 peak;
+`cpu_baseline` = the fp64 oracle timed on this box's host cores on a bounded sample of the workload.
+Multi-GPU (torchrun): rows are independent problems -> each rank runs its own batch, no data-path
+collective (weak scaling); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import tri_inputs  # noqa: E402
+
+METRIC = "triangle-attn fwd+bwd TFLOP/s"
+UNIT = "TFLOP/s"
+SPEC_BF16_TFLOPS = 2250.0  # nominal dense bf16 (context only)
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def model_flop(cfg, rows=None) -> float:
+    """14*B*H*N^3*d for the full problem; `rows` = number of (b,row) slices if a sample."""
+    per_slice = 14.0 * cfg.H * cfg.N * cfg.N * cfg.d
+    n = cfg.B * cfg.N if rows is None else rows
+    return per_slice * n
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {k: float(d[k]) for k in FALLBACK_PEAKS if k in d} | {"source": "measured"}
+    return dict(FALLBACK_PEAKS, source="fallback")
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks sampling (nvidia-smi in the background during the timed region)
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline of our arm, and the whole of --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_inputs(cfg, rows_per_batch: int):
+    """`rows_per_batch` broadcast rows of the workload (rows are independent given the bias plane), same
+    distributions / rounding / mask recipe as tri_inputs.make_inputs, expressed in starting-node form."""
+    rng = np.random.Generator(np.random.Philox(cfg.seed + 77))
+    B, N, H, d, R = cfg.B, cfg.N, cfg.H, cfg.d, rows_per_batch
+    x = {k: rng.standard_normal((B, R, H, N, d), dtype=np.float32) for k in ("Q", "K", "V", "G", "dO")}
+    x["bias"] = rng.standard_normal((B, H, N, N), dtype=np.float32) * np.float32(cfg.sigma_bias)
+    keep = tri_inputs.key_keep(cfg, rng)
+    x["mask"] = None if keep is None else np.ascontiguousarray(np.broadcast_to(keep[:, None, :], (B, R, N)))
+    if cfg.dtype == "bf16":
+        for k in ("Q", "K", "V", "G", "dO", "bias"):
+            x[k] = tri_inputs.round_bf16(x[k])
+    return x
+
+
+def time_oracle(cfg, rows_per_batch: int, reps: int = 1):
+    """Seconds per pass of the fp64 oracle (fwd + bwd) over the sample; returns (sec, flop, threads)."""
+    import oracle
+
+    oracle.build()
+    x = oracle_sample_inputs(cfg, rows_per_batch)
+    x64 = {k: (None if v is None else (v if v.dtype == np.uint8 else v.astype(np.float64))) for k, v in x.items()}
+    best = float("inf")
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.fwd_start_general(x64["Q"], x64["K"], x64["V"], x64["G"], x64["bias"], x64["mask"])
+        oracle.bwd_start_general(x64["dO"], x64["Q"], x64["K"], x64["V"], x64["G"], x64["bias"], x64["mask"])
+        best = min(best, time.perf_counter() - t0)
+    return best, model_flop(cfg, rows=cfg.B * rows_per_batch), oracle.num_threads()
+
+
+def oracle_rows_for_budget(cfg, seconds: float) -> int:
+    """Pick a row count so one oracle pass takes about `seconds` (calibrated on an 8-row pass)."""
+    t8, _, _ = time_oracle(cfg, 8)
+    return int(max(1, min(cfg.N, 8 * seconds / max(t8, 1e-4))))
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    total_budget = 120.0  # seconds for warmup+steps
+    per_step = total_budget / max(1, args.steps + args.warmup)
+    R = oracle_rows_for_budget(cfg, min(per_step, 20.0))
+    for _ in range(args.warmup):
+        time_oracle(cfg, R)
+    t, fl, thr = 0.0, 0.0, 1
+    for _ in range(args.steps):
+        s, f, thr = time_oracle(cfg, R)
+        t += s
+        fl += f
+    val = fl / t / 1e12
+    sample = f"{R} of {cfg.N} broadcast rows per batch element (B={cfg.B}), full key range, fwd+bwd, fp64"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_name(cfg) -> str:
+    v = "starting" if cfg.variant == tri_inputs.STARTING else "ending"
+    return (f"{cfg.name}: triangle attention {v} node, {cfg.dtype}, B={cfg.B} N={cfg.N} H={cfg.H} d={cfg.d}, "
+            f"bias sigma={cfg.sigma_bias}, mask={cfg.mask}, seed={cfg.seed}")
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+# executed tensor FLOP per logit-pass of each kernel, in units of B*H*N^3*d (2 per matmul)
+KERNEL_FLOP_UNITS = (("fwd", 4.0), ("dkdv", 8.0), ("dq", 6.0), ("dbias", 4.0))
+
+
+def kernel_flop(name: str, cfg) -> float | None:
+    base = float(cfg.B) * cfg.H * cfg.N ** 3 * cfg.d
+    for key, units in KERNEL_FLOP_UNITS:
+        if key in name:
+            return units * base
+    return None
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2506_20686_b200 as tri
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU path; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    tri.load()
+    peaks = load_peaks()
+
+    # ---- inputs: seeded synthetic, rounded to bf16 once; each rank draws its own batch (weak scaling)
+    rcfg = tri_inputs.Config(**{**cfg.__dict__, "seed": cfg.seed + 1000 * rank})
+    x = tri_inputs.make_inputs(rcfg)
+    tdt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
+    names = ("Q", "K", "V", "G", "bias", "dO")
+    host = {k: torch.from_numpy(x[k]).to(tdt).pin_memory() for k in names}
+    host["mask"] = None if x["mask"] is None else torch.from_numpy(x["mask"]).pin_memory()
+    del x
+    g = {k: (None if v is None else v.to(dev)) for k, v in host.items()}
+    B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
+    code = tri.BF16 if cfg.dtype == "bf16" else tri.F32
+    O = torch.empty_like(g["Q"])
+    LSE = torch.empty((B, N, H, N), dtype=torch.float32, device=dev)
+    grads = tuple(torch.empty_like(g["Q"]) for _ in range(4)) + (torch.empty((B, H, N, N), dtype=torch.float32, device=dev),)
+    ws_bytes = max(tri.fwd_workspace_bytes(B, N, H, d, cfg.variant, code), tri.bwd_workspace_bytes(B, N, H, d, cfg.variant, code))
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+
+    def step():
+        tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], cfg.variant, O=O, LSE=LSE, workspace=ws)
+        tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], O, LSE, cfg.variant, out=grads,
+                         workspace=ws)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    torch.cuda.reset_peak_memory_stats()
+
+    # ---- timed region: K steps, CUDA events on the launching stream, per-kernel events inside the library
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = tri.launch_count()
+    tri.profile_begin()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    prof = tri.profile_end()
+    launches = tri.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    peak_bytes = torch.cuda.max_memory_allocated()
+    if world > 1:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    flop_all = model_flop(cfg) * world
+    value = flop_all / (ms_step * 1e-3) / 1e12
+
+    # ---- e2e: the same step through tri_attn_step_host on pinned HOST buffers (H2D + D2H inside)
+    hout = {k: torch.empty_like(host["Q"]).pin_memory() for k in ("O", "dQ", "dK", "dV", "dG")}
+    hout["LSE"] = torch.empty((B, N, H, N), dtype=torch.float32).pin_memory()
+    hout["dBias"] = torch.empty((B, H, N, N), dtype=torch.float32).pin_memory()
+    del O, LSE, grads, ws, g
+    torch.cuda.empty_cache()
+    arena = torch.empty(tri.step_host_arena_bytes(B, N, H, d, cfg.variant, code), dtype=torch.uint8, device=dev)
+    hin = dict(host)
+    e2e_steps = max(2, min(args.steps, 5))
+    tri.tri_attn_step_host(hin, hout, cfg.variant, arena)  # warm-up
+    barrier()
+    e0.record()
+    for _ in range(e2e_steps):
+        tri.tri_attn_step_host(hin, hout, cfg.variant, arena)
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1) / e2e_steps
+    if world > 1:
+        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    h2d = sum(v.numel() * v.element_size() for v in hin.values() if v is not None)
+    d2h = sum(v.numel() * v.element_size() for v in hout.values())
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel
+    tot = sum(ms for _, ms in prof.values()) or 1.0
+    kernels = {k: {"launches": n, "ms_per_launch": ms / n, "share": ms / tot} for k, (n, ms) in prof.items()}
+    dom = max(prof, key=lambda k: prof[k][1])
+    dn, dms = prof[dom]
+    dflop = kernel_flop(dom, cfg)
+    sustained = args.steps * ms_step > 500.0  # a long step loop sits under the power cap
+    peak = peaks["bf16_tflops_sustained" if sustained else "bf16_tflops"]
+    if dflop is not None:
+        ach = dflop / (dms / dn * 1e-3) / 1e12
+        bound = "tensor" if "simt" not in dom else "alu"
+        if bound == "alu":
+            # fp32 CUDA-core kernels: 148 SMs x 128 FMA lanes x 2 flop x max SM clock
+            peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        roof = {"kernel": dom, "bound": bound, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": None, "peak_source": peaks["source"] + (" sustained" if sustained else " burst") if bound == "tensor"
+                else "derived: 148 SM x 128 lanes x 2 x 1.965 GHz", "flop_per_launch": dflop, "ms_per_launch": dms / dn}
+    else:
+        U = B * N * H * N * d * (2 if cfg.dtype == "bf16" else 4)
+        bytes_ = 4 * U + B * N * H * N * 4  # preprocess: read dO,O,G, write dG + D
+        ach = bytes_ / (dms / dn * 1e-3) / 1e9
+        roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]}
+
+    # ---- oracle on the host cores, bounded sample (~15 s)
+    R = oracle_rows_for_budget(cfg, 15.0 / 1.0)
+    sec, fl, thr = time_oracle(cfg, R)
+    cpu = {"value": fl / sec / 1e12, "unit": UNIT, "cores": thr, "kind": "oracle",
+           "sample": f"{R} of {N} broadcast rows per batch element (B={B}), full key range, fwd+bwd fp64, {sec:.1f} s"}
+
+    U_bytes = B * N * H * N * d * (2 if cfg.dtype == "bf16" else 4)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
+        "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "per_gpu_batch": B, "l2": "inputs (10 x %.0f MB) exceed the 126 MB L2; no flush" % (U_bytes / 1e6),
+                   "model_flop_per_step_per_gpu": model_flop(cfg)},
+        "pct_of_peak": {"spec_2250": 100 * value / world / SPEC_BF16_TFLOPS,
+                        "measured_burst": 100 * value / world / peaks["bf16_tflops"],
+                        "measured_sustained": 100 * value / world / peaks["bf16_tflops_sustained"], "peaks": peaks["source"]},
+        "memory": {"peak_gb": peak_bytes / 1e9, "io_tensors_gb": (10 * U_bytes + 3 * B * H * N * N * 4) / 1e9,
+                   "workspace_bytes": ws_bytes, "avoided_map_gb_bf16": B * H * N ** 3 * 2 / 1e9},
+        "kernels": kernels, "roofline": roof, "cpu_baseline": cpu,
+        "e2e": {"value": flop_all / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": ms_e2e,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(tri_inputs.CONFIGS))
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = tri_inputs.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

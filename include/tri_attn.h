@@ -109,6 +109,14 @@ TRI_API tri_status tri_attn_step_host(const void* hQ, const void* hK, const void
 /* Number of kernel launches this library has enqueued since it was loaded (for bench accounting). */
 TRI_API unsigned long long tri_attn_launch_count(void);
 
+/* Per-kernel timing for the bench's roofline line.  After _begin, every kernel the library launches is
+ * bracketed by CUDA events on its stream.  _end synchronises those events (the only call here that
+ * blocks the host), stops recording and writes one text line per kernel name into `buf` (host):
+ * "<kernel> <launches> <total_ms>\n".  Returns the number of distinct kernels, -1 on a CUDA error.
+ * Not thread-safe; at most 8192 launches are recorded per _begin. */
+TRI_API void tri_attn_profile_begin(void);
+TRI_API int tri_attn_profile_end(char* buf, size_t buflen);
+
 /* Static description of a status code. */
 TRI_API const char* tri_status_string(tri_status s);
 

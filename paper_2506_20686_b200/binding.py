@@ -29,6 +29,8 @@ SIGNATURES = {
     "tri_attn_step_host_arena_bytes": (_sz, [_i] * 6),
     "tri_attn_step_host": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_launch_count": (ctypes.c_ulonglong, []),
+    "tri_attn_profile_begin": (None, []),
+    "tri_attn_profile_end": (_i, [ctypes.c_char_p, _sz]),
     "tri_status_string": (ctypes.c_char_p, [_i]),
     "tri_attn_last_cuda_error": (ctypes.c_char_p, []),
 }
@@ -100,6 +102,24 @@ def bwd_workspace_bytes(B, N, H, d, variant, dtype_code) -> int:
 
 def launch_count() -> int:
     return int(load().tri_attn_launch_count())
+
+
+def profile_begin() -> None:
+    """Start bracketing every kernel the library launches with CUDA events (bench roofline leg)."""
+    load().tri_attn_profile_begin()
+
+
+def profile_end() -> dict:
+    """Stop, synchronise the events and return {kernel_name: (launches, total_ms)}."""
+    buf = ctypes.create_string_buffer(1 << 14)
+    n = load().tri_attn_profile_end(buf, len(buf))
+    if n < 0:
+        raise TriAttnError("tri_attn_profile_end: CUDA error")
+    out = {}
+    for line in buf.value.decode().splitlines():
+        name, cnt, ms = line.split()
+        out[name] = (int(cnt), float(ms))
+    return out
 
 
 def _workspace(nbytes, device, workspace):

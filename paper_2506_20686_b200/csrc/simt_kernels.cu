@@ -313,8 +313,10 @@ template <typename T, int D>
 tri_status fwd_t(const Problem& p, const void* Q, const void* K, const void* V, const void* G, const void* bias,
                  const unsigned char* mask, void* O, float* LSE, cudaStream_t st) {
     dim3 grid(p.B * p.N * p.H, (p.N + 63) / 64);
+    { ProfScope ps("simt_fwd_kernel", st);
     simt_fwd_kernel<T, D><<<grid, 64, 0, st>>>(p, (const T*)Q, (const T*)K, (const T*)V, (const T*)G, (const T*)bias, mask,
                                                (T*)O, LSE);
+    }
     TRI_LAUNCH_CHECK("simt_fwd_kernel");
     return TRI_OK;
 }
@@ -325,19 +327,27 @@ tri_status bwd_t(const Problem& p, const void* dO, const void* Q, const void* K,
                  void* dV, void* dG, float* dBias, void* ws, cudaStream_t st) {
     float* Dws = (float*)ws;
     const long long rows = (long long)p.B * p.N * p.H * p.N;
+    { ProfScope ps("simt_preprocess_kernel", st);
     simt_preprocess_kernel<T, D><<<(unsigned)((rows + 127) / 128), 128, 0, st>>>(rows, (const T*)dO, (const T*)O,
                                                                                 (const T*)G, (T*)dG, Dws);
+    }
     TRI_LAUNCH_CHECK("simt_preprocess_kernel");
     dim3 grid(p.B * p.N * p.H, (p.N + 63) / 64);
+    { ProfScope ps("simt_dkdv_kernel", st);
     simt_dkdv_kernel<T, D><<<grid, 64, 0, st>>>(p, (const T*)dO, (const T*)Q, (const T*)K, (const T*)V, (const T*)G,
                                                 (const T*)bias, mask, LSE, Dws, (T*)dK, (T*)dV);
+    }
     TRI_LAUNCH_CHECK("simt_dkdv_kernel");
+    { ProfScope ps("simt_dq_kernel", st);
     simt_dq_kernel<T, D><<<grid, 64, 0, st>>>(p, (const T*)dO, (const T*)Q, (const T*)K, (const T*)V, (const T*)G,
                                               (const T*)bias, mask, LSE, Dws, (T*)dQ);
+    }
     TRI_LAUNCH_CHECK("simt_dq_kernel");
     dim3 gb((p.N + 15) / 16, (p.N + 15) / 16, p.B * p.H);
+    { ProfScope ps("simt_dbias_kernel", st);
     simt_dbias_kernel<T, D><<<gb, 256, 0, st>>>(p, (const T*)dO, (const T*)Q, (const T*)K, (const T*)V, (const T*)G,
                                                 (const T*)bias, mask, LSE, Dws, dBias);
+    }
     TRI_LAUNCH_CHECK("simt_dbias_kernel");
     return TRI_OK;
 }

@@ -18,6 +18,31 @@ tri_status cuda_fail(cudaError_t e, const char* where) {
     return TRI_ERR_CUDA;
 }
 
+// ---- per-kernel event timing --------------------------------------------------------------------
+namespace {
+struct ProfRec { const char* name; cudaEvent_t a, b; };
+constexpr int kMaxProf = 8192;
+ProfRec g_prof[kMaxProf];
+int g_prof_n = 0;
+int g_prof_created = 0;
+bool g_prof_on = false;
+}  // namespace
+
+ProfScope::ProfScope(const char* name, cudaStream_t s) : idx(-1), st(s) {
+    if (!g_prof_on || g_prof_n >= kMaxProf) return;
+    idx = g_prof_n++;
+    if (idx >= g_prof_created) {
+        cudaEventCreate(&g_prof[idx].a);
+        cudaEventCreate(&g_prof[idx].b);
+        g_prof_created = idx + 1;
+    }
+    g_prof[idx].name = name;
+    cudaEventRecord(g_prof[idx].a, st);
+}
+ProfScope::~ProfScope() {
+    if (idx >= 0) cudaEventRecord(g_prof[idx].b, st);
+}
+
 static bool shape_ok(int B, int N, int H, int d) { return B > 0 && N > 0 && H > 0 && d > 0; }
 static bool enums_ok(int variant, int dtype) {
     return (variant == TRI_STARTING || variant == TRI_ENDING) && (dtype == TRI_F32 || dtype == TRI_BF16);
@@ -163,6 +188,39 @@ tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, co
     for (int i = 0; i < 4; ++i) TRI_CUDA_CHECK(cudaMemcpyAsync(hout[i], dout[i], Ub, cudaMemcpyDeviceToHost, st));
     TRI_CUDA_CHECK(cudaMemcpyAsync(hdBias, gBias, (size_t)B * H * N * N * 4, cudaMemcpyDeviceToHost, st));
     return TRI_OK;
+}
+
+void tri_attn_profile_begin(void) {
+    g_prof_n = 0;
+    g_prof_on = true;
+}
+
+int tri_attn_profile_end(char* buf, size_t buflen) {
+    g_prof_on = false;
+    struct Agg { const char* name; int n; double ms; } agg[64];
+    int na = 0;
+    for (int i = 0; i < g_prof_n; ++i) {
+        if (cudaEventSynchronize(g_prof[i].b) != cudaSuccess) return -1;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, g_prof[i].a, g_prof[i].b) != cudaSuccess) return -1;
+        int j = 0;
+        while (j < na && strcmp(agg[j].name, g_prof[i].name) != 0) ++j;
+        if (j == na) {
+            if (na == 64) continue;
+            agg[na++] = Agg{g_prof[i].name, 0, 0.0};
+        }
+        agg[j].n += 1;
+        agg[j].ms += ms;
+    }
+    size_t off = 0;
+    if (buf && buflen) buf[0] = 0;
+    for (int j = 0; j < na && buf; ++j) {
+        int w = snprintf(buf + off, off < buflen ? buflen - off : 0, "%s %d %.6f\n", agg[j].name, agg[j].n, agg[j].ms);
+        if (w < 0 || off + (size_t)w >= buflen) break;
+        off += (size_t)w;
+    }
+    g_prof_n = 0;
+    return na;
 }
 
 unsigned long long tri_attn_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

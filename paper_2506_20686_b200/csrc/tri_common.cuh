@@ -63,6 +63,15 @@ tri_status cuda_fail(cudaError_t e, const char* where);
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Per-kernel CUDA-event timing (tri_attn_profile_begin / _end in the ABI).  Declare one in the scope
+// of a launch: records an event before and after it on `st` while profiling is on, else does nothing.
+struct ProfScope {
+    ProfScope(const char* name, cudaStream_t st);
+    ~ProfScope();
+    int idx;
+    cudaStream_t st;
+};
+
 // ---- fp32 CUDA-core path (simt_kernels.cu) -------------------------------------------------
 size_t simt_fwd_workspace(const Problem& p);
 size_t simt_bwd_workspace(const Problem& p);
