@@ -8,6 +8,8 @@
 //   x = scale*S + bias (+ -inf mask); online max / sum; p = exp2((x - m) log2e)
 //   P -> bf16 -> TMEM (aliases S);  O_r += P V_r   tcgen05.mma TS, M=128 N=32 K=8x16, V MN-major
 // Epilogue: O = sigmoid(G) * O_r / l, LSE = m + ln l.
+#include <stdlib.h>
+
 #include "sm100_common.cuh"
 #include "tri_common.cuh"
 
@@ -315,7 +317,9 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK) ||
         !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane(&tB, bias_qk, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
-    return launch_fwd<4>(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
+    static const bool v1 = getenv("TRI_FWD_V1") != nullptr;
+    if (v1) return launch_fwd<4>(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
+    return sm100_fwd2_launch(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
 }
 
 }  // namespace tri
