@@ -69,7 +69,7 @@ struct DkdvSmem {
 };
 
 template <int R_>
-__global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__ CUtensorMap tmQ64,
+__global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constant__ CUtensorMap tmQ64,
                                                          const __grid_constant__ CUtensorMap tmA64,
                                                          const __grid_constant__ CUtensorMap tmK128,
                                                          const __grid_constant__ CUtensorMap tmV128,
@@ -92,7 +92,9 @@ __global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__
     uint64_t* bar_mma = bars + 4;
     uint32_t* tmem_slot = (uint32_t*)(bars + 5);
 
-    const int tid = threadIdx.x, warp = tid >> 5;
+    // 256 threads: a key row (TMEM lane) is shared by two threads, warps w and w+4, 32 query columns each
+    const int tid = threadIdx.x, warp = tid >> 5, chalf = warp >> 2;
+    const int row = (warp & 3) * 32 + (tid & 31);
     const int NKB = p.N / 128, NQT = p.N / 64, NG = p.N / R_;
     int idx = blockIdx.x;
     const int kb = idx % NKB; idx /= NKB;
@@ -111,7 +113,7 @@ __global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t lane_off = (uint32_t)(warp * 32) << 16;
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t tS = tmem, tDP = tmem + 64;
     const int T = NQT * R_;
 
@@ -139,18 +141,19 @@ __global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__
             const float l = __ldg(LSE + o);
             return l == -INFINITY ? -INFINITY : -l * kLog2e;
         }
-        return __ldg(Dws + o);
+        return -__ldg(Dws + o);
     };
-    sLD[tid] = ld_val(0);
+    if (tid < 128) sLD[tid] = ld_val(0);
     bool keep[R_];
 #pragma unroll
     for (int r = 0; r < R_; ++r)
-        keep[r] = !mask || mask[(long long)b * p.N * p.N + (long long)(r0 + r) * p.mR + (long long)(k0 + tid) * p.mK];
+        keep[r] = !mask || mask[(long long)b * p.N * p.N + (long long)(r0 + r) * p.mR + (long long)(k0 + row) * p.mK];
     __syncthreads();
 
     constexpr uint32_t idescS = make_idesc(128, 64, false, false);
     constexpr uint32_t idescO = make_idesc(128, DH, false, true);
     const float scale = rsqrtf((float)DH);
+    const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
 
     for (int qt = 0; qt < NQT; ++qt) {
 #pragma unroll
@@ -171,43 +174,53 @@ __global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__
                 mma_commit(bar_mma);
             }
             float ldnext = 0.0f;
-            if (t + 1 < T) ldnext = ld_val(t + 1);
+            if (t + 1 < T && tid < 128) ldnext = ld_val(t + 1);
             mbar_wait(bar_mma, t & 1);
             tc_fence_after();
             if (tid == 0 && t + 1 < T) load_qa(t + 1);
             if (r == 0) mbar_wait(bar_bias, qt & 1);
             const float* nlq = sLD + st * 128;
             const float* ddq = nlq + 64;
-#pragma unroll
-            for (int c32 = 0; c32 < 2; ++c32) {
+            {
+                const int c32 = chalf;
                 uint32_t sraw[32], dpraw[32];
                 tmem_ld32(tS + lane_off + c32 * 32, sraw);
                 tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
                 uint4 bv[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sBias + tid * 128 + (((c32 * 4 + j) ^ (tid & 7)) << 4));
+                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sBias + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
                 tmem_ld_wait();
                 uint32_t pp[16], ds[16];
+                if (keep[r]) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const uint32_t w[4] = {bv[j].x, bv[j].y, bv[j].z, bv[j].w};
+                    for (int j = 0; j < 4; ++j) {
+                        const uint32_t w[4] = {bv[j].x, bv[j].y, bv[j].z, bv[j].w};
+                        const float4 n0 = *(const float4*)(nlq + c32 * 32 + j * 8), n1 = *(const float4*)(nlq + c32 * 32 + j * 8 + 4);
+                        const float4 d0 = *(const float4*)(ddq + c32 * 32 + j * 8), d1 = *(const float4*)(ddq + c32 * 32 + j * 8 + 4);
+                        const uint64_t nn[4] = {pack2(n0.x, n0.y), pack2(n0.z, n0.w), pack2(n1.x, n1.y), pack2(n1.z, n1.w)};
+                        const uint64_t dn[4] = {pack2(d0.x, d0.y), pack2(d0.z, d0.w), pack2(d1.x, d1.y), pack2(d1.z, d1.w)};
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int c = j * 8 + e * 2, q = c32 * 32 + c;
-                        float x0 = fmaf(__uint_as_float(sraw[c]), scale, bf16_lo(w[e]));
-                        float x1 = fmaf(__uint_as_float(sraw[c + 1]), scale, bf16_hi(w[e]));
-                        if (!keep[r]) { x0 = -INFINITY; x1 = -INFINITY; }
-                        const float p0 = ex2(fmaf(x0, kLog2e, nlq[q])), p1 = ex2(fmaf(x1, kLog2e, nlq[q + 1]));
-                        const float s0 = p0 * (__uint_as_float(dpraw[c]) - ddq[q]);
-                        const float s1 = p1 * (__uint_as_float(dpraw[c + 1]) - ddq[q + 1]);
-                        pp[j * 4 + e] = pack_bf16(p0, p1);
-                        ds[j * 4 + e] = pack_bf16(s0, s1);
+                        for (int e = 0; e < 4; ++e) {
+                            const int c = j * 8 + e * 2;
+                            const uint64_t x2 = fma2(pack2(__uint_as_float(sraw[c]), __uint_as_float(sraw[c + 1])), scale2,
+                                                     pack2(bf16_lo(w[e]), bf16_hi(w[e])));
+                            float a0, a1, s0, s1;
+                            unpack2(fma2(x2, l2e2, nn[e]), a0, a1);
+                            const float p0 = ex2(a0), p1 = ex2(a1);
+                            // sLD holds -D: ds = p * (dp - D)
+                            unpack2(mul2(pack2(p0, p1), add2(pack2(__uint_as_float(dpraw[c]), __uint_as_float(dpraw[c + 1])), dn[e])), s0, s1);
+                            pp[j * 4 + e] = pack_bf16(p0, p1);
+                            ds[j * 4 + e] = pack_bf16(s0, s1);
+                        }
                     }
+                } else {  // masked key: its whole row of P^T and dS^T is zero
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) { pp[e] = 0u; ds[e] = 0u; }
                 }
-                tmem_st16(tS + lane_off + c32 * 16, pp);
-                tmem_st16(tDP + lane_off + c32 * 16, ds);
+                tmem_st16(tS + lane_off + c32 * 32, pp);   // packed into my own fp32 columns [32*c32, +16)
+                tmem_st16(tDP + lane_off + c32 * 32, ds);
             }
-            if (t + 1 < T) sLD[((t + 1) & 1) * 128 + tid] = ldnext;
+            if (t + 1 < T && tid < 128) sLD[((t + 1) & 1) * 128 + tid] = ldnext;
             tmem_st_wait();
             tc_fence_before();
             __syncthreads();
@@ -217,9 +230,11 @@ __global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__
                 const uint64_t da = make_desc_sw64(smem_u32(sQA + st * 2 * T64 + T64));
                 const uint32_t tdV = tmem + 128 + r * 64, tdK = tdV + 32;
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks) mma_ts(tdV, tS + ks * 8, da + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
+                for (int ks = 0; ks < 4; ++ks)  // A columns: k-steps 0,1 at [0,16), k-steps 2,3 at [32,48)
+                    mma_ts(tdV, tS + (ks >> 1) * 32 + (ks & 1) * 8, da + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks) mma_ts(tdK, tDP + ks * 8, dq + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
+                for (int ks = 0; ks < 4; ++ks)
+                    mma_ts(tdK, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dq + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
                 if (r == R_ - 1 && qt + 1 < NQT) {
                     mbar_expect_tx(bar_bias, 16384);
                     tma_load_3d(sBias, &tmBiasKQ, bar_bias, (qt + 1) * 64, k0, bh);
@@ -231,24 +246,20 @@ __global__ void __launch_bounds__(128) sm100_dkdv_kernel(const __grid_constant__
     mbar_wait(bar_mma, T & 1);
     tc_fence_after();
 #pragma unroll
-    for (int r = 0; r < R_; ++r) {
-        uint32_t v[32], k[32];
-        tmem_ld32(tmem + lane_off + 128 + r * 64, v);
-        tmem_ld32(tmem + lane_off + 128 + r * 64 + 32, k);
+    for (int r = 0; r < R_; ++r) {  // warps 0-3 write dV_r, warps 4-7 write dK_r (scaled)
+        uint32_t v[32];
+        tmem_ld32(tmem + lane_off + 128 + r * 64 + chalf * 32, v);
         tmem_ld_wait();
-        const long long off = (long long)b * p.sB + (long long)h * p.sH + (long long)(r0 + r) * p.sSlice + (long long)(k0 + tid) * p.sPos;
-        uint4* pv = (uint4*)(dV + off);
-        uint4* pk = (uint4*)(dK + off);
+        const long long off = (long long)b * p.sB + (long long)h * p.sH + (long long)(r0 + r) * p.sSlice + (long long)(k0 + row) * p.sPos;
+        uint4* po = (uint4*)((chalf ? dK : dV) + off);
+        const float sc = chalf ? scale : 1.0f;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            uint32_t a[4], c[4];
+            uint32_t a[4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                a[e] = pack_bf16(__uint_as_float(v[j * 8 + 2 * e]), __uint_as_float(v[j * 8 + 2 * e + 1]));
-                c[e] = pack_bf16(__uint_as_float(k[j * 8 + 2 * e]) * scale, __uint_as_float(k[j * 8 + 2 * e + 1]) * scale);
-            }
-            pv[j] = make_uint4(a[0], a[1], a[2], a[3]);
-            pk[j] = make_uint4(c[0], c[1], c[2], c[3]);
+            for (int e = 0; e < 4; ++e)
+                a[e] = pack_bf16(__uint_as_float(v[j * 8 + 2 * e]) * sc, __uint_as_float(v[j * 8 + 2 * e + 1]) * sc);
+            po[j] = make_uint4(a[0], a[1], a[2], a[3]);
         }
     }
     tc_fence_before();
@@ -270,7 +281,7 @@ struct DqSmem {
 };
 
 template <int R_>
-__global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ CUtensorMap tmQ128,
+__global__ void __launch_bounds__(256, 2) sm100_dq_kernel(const __grid_constant__ CUtensorMap tmQ128,
                                                        const __grid_constant__ CUtensorMap tmA128,
                                                        const __grid_constant__ CUtensorMap tmK64,
                                                        const __grid_constant__ CUtensorMap tmV64,
@@ -293,7 +304,9 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
     uint64_t* bar_mma = bars + 4;
     uint32_t* tmem_slot = (uint32_t*)(bars + 5);
 
-    const int tid = threadIdx.x, warp = tid >> 5;
+    // 256 threads: a query row (TMEM lane) is shared by two threads, warps w and w+4, 32 key columns each
+    const int tid = threadIdx.x, warp = tid >> 5, chalf = warp >> 2;
+    const int row = (warp & 3) * 32 + (tid & 31);
     const int NQB = p.N / 128, NKT = p.N / 64, NG = p.N / R_;
     int idx = blockIdx.x;
     const int qb = idx % NQB; idx /= NQB;
@@ -312,7 +325,7 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t lane_off = (uint32_t)(warp * 32) << 16;
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t tS = tmem, tDP = tmem + 64;
     const int T = NKT * R_;
 
@@ -346,7 +359,7 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
     float nl[R_], dd[R_];
 #pragma unroll
     for (int r = 0; r < R_; ++r) {
-        const long long o = (long long)b * p.N * p.H * p.N + (long long)h * p.N + (long long)(r0 + r) * p.lR + (long long)(q0 + tid) * p.lQ;
+        const long long o = (long long)b * p.N * p.H * p.N + (long long)h * p.N + (long long)(r0 + r) * p.lR + (long long)(q0 + row) * p.lQ;
         const float l = __ldg(LSE + o);
         nl[r] = l == -INFINITY ? -INFINITY : -l * kLog2e;
         dd[r] = __ldg(Dws + o);
@@ -355,6 +368,7 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
     constexpr uint32_t idescS = make_idesc(128, 64, false, false);
     constexpr uint32_t idescO = make_idesc(128, DH, false, true);
     const float scale = rsqrtf((float)DH);
+    const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
 
     for (int kt = 0; kt < NKT; ++kt) {
 #pragma unroll
@@ -381,30 +395,43 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
             if (tid == 0 && t + 1 < T) load_kv(t + 1);
             if (r == 0) mbar_wait(bar_bias, kt & 1);
             const float* mrow = sMask + st * 64;
-#pragma unroll
-            for (int c32 = 0; c32 < 2; ++c32) {
+            {
+                const int c32 = chalf;
                 uint32_t sraw[32], dpraw[32];
                 tmem_ld32(tS + lane_off + c32 * 32, sraw);
                 tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
                 uint4 bv[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sBias + tid * 128 + (((c32 * 4 + j) ^ (tid & 7)) << 4));
+                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sBias + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
                 tmem_ld_wait();
                 uint32_t ds[16];
+                if (anymask) {
+#pragma unroll
+                    for (int c4 = 0; c4 < 8; ++c4) {
+                        const float4 mv = *(const float4*)(mrow + c32 * 32 + c4 * 4);
+                        sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);  // -inf survives the scale
+                        sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
+                        sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);
+                        sraw[c4 * 4 + 3] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 3]) + mv.w);
+                    }
+                }
+                const uint64_t nl2 = pack2(nl[r], nl[r]), nd2 = pack2(-dd[r], -dd[r]);
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const uint32_t w[4] = {bv[j].x, bv[j].y, bv[j].z, bv[j].w};
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
-                        const int c = j * 8 + e * 2, k = c32 * 32 + c;
-                        float x0 = fmaf(__uint_as_float(sraw[c]), scale, bf16_lo(w[e]));
-                        float x1 = fmaf(__uint_as_float(sraw[c + 1]), scale, bf16_hi(w[e]));
-                        if (anymask) { x0 += mrow[k]; x1 += mrow[k + 1]; }
-                        const float p0 = ex2(fmaf(x0, kLog2e, nl[r])), p1 = ex2(fmaf(x1, kLog2e, nl[r]));
-                        ds[j * 4 + e] = pack_bf16(p0 * (__uint_as_float(dpraw[c]) - dd[r]), p1 * (__uint_as_float(dpraw[c + 1]) - dd[r]));
+                        const int c = j * 8 + e * 2;
+                        const uint64_t x2 = fma2(pack2(__uint_as_float(sraw[c]), __uint_as_float(sraw[c + 1])), scale2,
+                                                 pack2(bf16_lo(w[e]), bf16_hi(w[e])));
+                        float a0, a1, s0, s1;
+                        unpack2(fma2(x2, l2e2, nl2), a0, a1);
+                        const float p0 = ex2(a0), p1 = ex2(a1);
+                        unpack2(mul2(pack2(p0, p1), add2(pack2(__uint_as_float(dpraw[c]), __uint_as_float(dpraw[c + 1])), nd2)), s0, s1);
+                        ds[j * 4 + e] = pack_bf16(s0, s1);
                     }
                 }
-                tmem_st16(tDP + lane_off + c32 * 16, ds);
+                tmem_st16(tDP + lane_off + c32 * 32, ds);
             }
             if (mask && t + 1 < T && tid < 64) sMask[((t + 1) & 1) * 64 + tid] = mnext;
             tmem_st_wait();
@@ -415,7 +442,8 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
                 const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * T64));
 #pragma unroll
                 for (int ks = 0; ks < 4; ++ks)
-                    mma_ts(tmem + 128 + r * 32, tDP + ks * 8, dk + (uint64_t)ks * 64, idescO, (kt > 0 || ks > 0) ? 1u : 0u);
+                    mma_ts(tmem + 128 + r * 32, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dk + (uint64_t)ks * 64, idescO,
+                           (kt > 0 || ks > 0) ? 1u : 0u);
                 if (r == R_ - 1 && kt + 1 < NKT) {
                     mbar_expect_tx(bar_bias, 16384);
                     tma_load_3d(sBias, &tmBiasQK, bar_bias, (kt + 1) * 64, q0, bh);
@@ -427,11 +455,11 @@ __global__ void __launch_bounds__(128) sm100_dq_kernel(const __grid_constant__ C
     mbar_wait(bar_mma, T & 1);
     tc_fence_after();
 #pragma unroll
-    for (int r = 0; r < R_; ++r) {
+    for (int r = chalf * (R_ / 2); r < (chalf + 1) * (R_ / 2); ++r) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_off + 128 + r * 32, v);
         tmem_ld_wait();
-        const long long off = (long long)b * p.sB + (long long)h * p.sH + (long long)(r0 + r) * p.sSlice + (long long)(q0 + tid) * p.sPos;
+        const long long off = (long long)b * p.sB + (long long)h * p.sH + (long long)(r0 + r) * p.sSlice + (long long)(q0 + row) * p.sPos;
         uint4* pq = (uint4*)(dQ + off);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -550,15 +578,17 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
     if (tid == 0) issue_mma(0);
     float lse_n = __ldg(LSE + lse_off(0)), dd_n = __ldg(Dws + lse_off(0));
     const float scale = rsqrtf((float)DH);
-    float acc[64];
+    uint64_t acc2[32];  // dBias tile: my 64 columns as fp32 pairs
 #pragma unroll
-    for (int c = 0; c < 64; ++c) acc[c] = 0.0f;
+    for (int c = 0; c < 32; ++c) acc2[c] = pack2(0.0f, 0.0f);
+    const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
     mbar_wait(bar_bias, 0);
 
     for (int r = 0; r < N; ++r) {
         const int j = r & 1;
         if (tid == 0 && r + 1 < N) issue_mma(r + 1);
         const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e, dd = dd_n;
+        const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd, -dd);
         float mnext = 0.0f;
         if (r + 1 < N) {
             lse_n = __ldg(LSE + lse_off(r + 1));
@@ -580,18 +610,27 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
             for (int jj = 0; jj < 4; ++jj)
                 bv[jj] = *(const uint4*)(sBias + half * 16384 + qrow * 128 + (((c32 * 4 + jj) ^ (qrow & 7)) << 4));
             tmem_ld_wait();
+            if (anymask) {
+#pragma unroll
+                for (int c4 = 0; c4 < 8; ++c4) {
+                    const float4 mv = *(const float4*)(mrow + c32 * 32 + c4 * 4);
+                    sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);
+                    sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
+                    sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);
+                    sraw[c4 * 4 + 3] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 3]) + mv.w);
+                }
+            }
 #pragma unroll
             for (int jj = 0; jj < 4; ++jj) {
                 const uint32_t w[4] = {bv[jj].x, bv[jj].y, bv[jj].z, bv[jj].w};
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const int c = jj * 8 + e * 2, k = c32 * 32 + c;
-                    float x0 = fmaf(__uint_as_float(sraw[c]), scale, bf16_lo(w[e]));
-                    float x1 = fmaf(__uint_as_float(sraw[c + 1]), scale, bf16_hi(w[e]));
-                    if (anymask) { x0 += mrow[k]; x1 += mrow[k + 1]; }
-                    const float p0 = ex2(fmaf(x0, kLog2e, nl)), p1 = ex2(fmaf(x1, kLog2e, nl));
-                    acc[k] = fmaf(p0, __uint_as_float(dpraw[c]) - dd, acc[k]);
-                    acc[k + 1] = fmaf(p1, __uint_as_float(dpraw[c + 1]) - dd, acc[k + 1]);
+                    const int c = jj * 8 + e * 2, k2 = (c32 * 32 + c) >> 1;
+                    const uint64_t x2 = fma2(pack2(__uint_as_float(sraw[c]), __uint_as_float(sraw[c + 1])), scale2,
+                                             pack2(bf16_lo(w[e]), bf16_hi(w[e])));
+                    float a0, a1;
+                    unpack2(fma2(x2, l2e2, nl2), a0, a1);
+                    acc2[k2] = fma2(pack2(ex2(a0), ex2(a1)), add2(pack2(__uint_as_float(dpraw[c]), __uint_as_float(dpraw[c + 1])), nd2), acc2[k2]);
                 }
             }
         }
@@ -600,6 +639,9 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         if (mask) anymask = __syncthreads_or(mnext != 0.0f); else __syncthreads();
     }
     float* out = dBias + (long long)bh * N * N + (long long)(q0 + qrow) * p.bQ + (long long)(k0 + half * 64) * p.bK;
+    float acc[64];
+#pragma unroll
+    for (int c = 0; c < 32; ++c) unpack2(acc2[c], acc[2 * c], acc[2 * c + 1]);
     if (p.bK == 1) {
 #pragma unroll
         for (int c = 0; c < 64; c += 4) *(float4*)(out + c) = make_float4(acc[c], acc[c + 1], acc[c + 2], acc[c + 3]);
@@ -676,14 +718,14 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     {
         ProfScope ps("sm100_dkdv_kernel", st);
         const unsigned grid = (unsigned)((long long)p.B * (p.N / RKV) * p.H * (p.N / 128));
-        sm100_dkdv_kernel<RKV><<<grid, 128, DkdvSmem<RKV>::total, st>>>(tQ64, tA64, tK128, tV128, tBkq, p, mask, LSE, Dws,
+        sm100_dkdv_kernel<RKV><<<grid, 256, DkdvSmem<RKV>::total, st>>>(tQ64, tA64, tK128, tV128, tBkq, p, mask, LSE, Dws,
                                                                        (__nv_bfloat16*)dK, (__nv_bfloat16*)dV);
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
     {
         ProfScope ps("sm100_dq_kernel", st);
         const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
-        sm100_dq_kernel<RQ><<<grid, 128, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
+        sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
                                                                  (__nv_bfloat16*)dQ);
     }
     TRI_LAUNCH_CHECK("sm100_dq_kernel");
