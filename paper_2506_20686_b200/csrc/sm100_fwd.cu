@@ -273,7 +273,7 @@ __global__ void transpose_bf16_kernel(const __nv_bfloat16* __restrict__ in, __nv
 }  // namespace
 
 tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cudaStream_t st) {
-    ProfScope ps("sm100_transpose_bf16", st);
+    ProfScope ps("transpose_bf16_kernel", st);
     transpose_bf16_kernel<<<dim3(N / 32, N / 32, BH), dim3(32, 8), 0, st>>>((const __nv_bfloat16*)in, (__nv_bfloat16*)out, N);
     return TRI_OK;
 }

@@ -331,11 +331,11 @@ tri_status sm100_fwd2_launch(const Problem& p, const CUtensorMap& tQ, const CUte
     }
     const unsigned grid = (unsigned)((long long)p.B * (p.N / RT) * p.H * (p.N / BQ));
     {
-        ProfScope ps("sm100_fwd_kernel", st);
+        ProfScope ps("sm100_fwd2_kernel", st);
         sm100_fwd2_kernel<<<grid, NTHREADS, F2Smem::total, st>>>(tQ, tK, tV, tB, p, (const __nv_bfloat16*)G, mask,
                                                                  (__nv_bfloat16*)O, LSE);
     }
-    TRI_LAUNCH_CHECK("sm100_fwd_kernel");
+    TRI_LAUNCH_CHECK("sm100_fwd2_kernel");
     return TRI_OK;
 }
 
