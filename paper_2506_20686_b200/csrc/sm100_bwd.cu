@@ -495,7 +495,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
                                                           const __grid_constant__ CUtensorMap tmBiasQK, Problem p,
                                                           const unsigned char* __restrict__ mask,
                                                           const float* __restrict__ LSE, const float* __restrict__ Dws,
-                                                          float* __restrict__ dBias) {
+                                                          float* __restrict__ dBias, float* __restrict__ planes, int G) {
     using L = DbiasSmem;
     constexpr int NST = L::NST;
     extern __shared__ uint8_t smem_raw[];
@@ -514,11 +514,14 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
     const int NT = p.N / 128;
     int idx = blockIdx.x;
     const int kt = idx % NT; idx /= NT;
-    const int qt = idx % NT;
-    const int bh = idx / NT;
+    const int qt = idx % NT; idx /= NT;
+    const int bh = idx % (p.B * p.H);
+    const int gi = idx / (p.B * p.H);  // which slice of the broadcast-row axis (G > 1 only to fill the SMs)
     const int b = bh / p.H, h = bh % p.H;
     const int q0 = qt * 128, k0 = kt * 128;
     const int N = p.N;
+    const int rows_per = (N + G - 1) / G, rb = gi * rows_per;
+    const int NR = min(rows_per, N - rb);  // this CTA sums rows rb .. rb+NR-1 in ascending order (r below is local)
 
     if (tid == 0) {
         prefetch_tmap(&tmQ128); prefetch_tmap(&tmA128); prefetch_tmap(&tmK128); prefetch_tmap(&tmV128); prefetch_tmap(&tmBiasQK);
@@ -536,10 +539,10 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         const int s = r % NST;
         uint8_t* base = sOp + s * 4 * T128;
         mbar_expect_tx(bar_full + s, 4 * T128);
-        tma_load_5d(base, &tmQ128, bar_full + s, 0, q0, r, h, b);
-        tma_load_5d(base + T128, &tmA128, bar_full + s, 0, q0, r, h, b);
-        tma_load_5d(base + 2 * T128, &tmK128, bar_full + s, 0, k0, r, h, b);
-        tma_load_5d(base + 3 * T128, &tmV128, bar_full + s, 0, k0, r, h, b);
+        tma_load_5d(base, &tmQ128, bar_full + s, 0, q0, rb + r, h, b);
+        tma_load_5d(base + T128, &tmA128, bar_full + s, 0, q0, rb + r, h, b);
+        tma_load_5d(base + 2 * T128, &tmK128, bar_full + s, 0, k0, rb + r, h, b);
+        tma_load_5d(base + 3 * T128, &tmV128, bar_full + s, 0, k0, rb + r, h, b);
     };
     constexpr uint32_t idescS = make_idesc(128, 128, false, false);
     auto issue_mma = [&](int r) {
@@ -557,17 +560,17 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         mma_commit(bar_mma + j);
     };
     if (tid == 0) {
-        for (int r = 0; r < NST && r < N; ++r) load_ops(r);
+        for (int r = 0; r < NST && r < NR; ++r) load_ops(r);
         mbar_expect_tx(bar_bias, 32768);
         tma_load_3d(sBias, &tmBiasQK, bar_bias, k0, q0, bh);
         tma_load_3d(sBias + 16384, &tmBiasQK, bar_bias, k0 + 64, q0, bh);
     }
     auto mask_val = [&](int r) -> float {
-        const unsigned char mk = mask[(long long)b * N * N + (long long)r * p.mR + (long long)(k0 + (tid & 127)) * p.mK];
+        const unsigned char mk = mask[(long long)b * N * N + (long long)(rb + r) * p.mR + (long long)(k0 + (tid & 127)) * p.mK];
         return mk ? 0.0f : -INFINITY;
     };
     auto lse_off = [&](int r) -> long long {
-        return (long long)b * N * p.H * N + (long long)h * N + (long long)r * p.lR + (long long)(q0 + qrow) * p.lQ;
+        return (long long)b * N * p.H * N + (long long)h * N + (long long)(rb + r) * p.lR + (long long)(q0 + qrow) * p.lQ;
     };
     int anymask = 0;
     if (mask) {
@@ -584,20 +587,20 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
     const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
     mbar_wait(bar_bias, 0);
 
-    for (int r = 0; r < N; ++r) {
+    for (int r = 0; r < NR; ++r) {
         const int j = r & 1;
-        if (tid == 0 && r + 1 < N) issue_mma(r + 1);
+        if (tid == 0 && r + 1 < NR) issue_mma(r + 1);
         const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e, dd = dd_n;
         const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd, -dd);
         float mnext = 0.0f;
-        if (r + 1 < N) {
+        if (r + 1 < NR) {
             lse_n = __ldg(LSE + lse_off(r + 1));
             dd_n = __ldg(Dws + lse_off(r + 1));
             if (mask) mnext = mask_val(r + 1);
         }
         mbar_wait(bar_mma + j, (r >> 1) & 1);
         tc_fence_after();
-        if (tid == 0 && r + NST < N) load_ops(r + NST);
+        if (tid == 0 && r + NST < NR) load_ops(r + NST);
         const uint32_t tS = tmem + j * 256 + half * 64, tDP = tS + 128;
         const float* mrow = sMask + j * 128 + half * 64;
 #pragma unroll
@@ -634,24 +637,51 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
                 }
             }
         }
-        if (mask && r + 1 < N && tid < 128) sMask[(j ^ 1) * 128 + tid] = mnext;
+        if (mask && r + 1 < NR && tid < 128) sMask[(j ^ 1) * 128 + tid] = mnext;
         tc_fence_before();
         if (mask) anymask = __syncthreads_or(mnext != 0.0f); else __syncthreads();
     }
-    float* out = dBias + (long long)bh * N * N + (long long)(q0 + qrow) * p.bQ + (long long)(k0 + half * 64) * p.bK;
     float acc[64];
 #pragma unroll
     for (int c = 0; c < 32; ++c) unpack2(acc2[c], acc[2 * c], acc[2 * c + 1]);
-    if (p.bK == 1) {
+    if (G > 1) {  // level-1 partial plane [gi][bh][q][k]; sm100_dbias_reduce_kernel adds the planes in ascending order
+        float* out = planes + ((long long)gi * p.B * p.H + bh) * N * N + (long long)(q0 + qrow) * N + k0 + half * 64;
 #pragma unroll
         for (int c = 0; c < 64; c += 4) *(float4*)(out + c) = make_float4(acc[c], acc[c + 1], acc[c + 2], acc[c + 3]);
     } else {
+        float* out = dBias + (long long)bh * N * N + (long long)(q0 + qrow) * p.bQ + (long long)(k0 + half * 64) * p.bK;
+        if (p.bK == 1) {
 #pragma unroll
-        for (int c = 0; c < 64; ++c) out[(long long)c * p.bK] = acc[c];
+            for (int c = 0; c < 64; c += 4) *(float4*)(out + c) = make_float4(acc[c], acc[c + 1], acc[c + 2], acc[c + 3]);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 64; ++c) out[(long long)c * p.bK] = acc[c];
+        }
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+
+// level 2 of the dBias reduction (only when the row axis was split): dBias[bh][q*bQ + k*bK] = sum over planes, in
+// ascending order, of plane[g][bh][q][k]; the ending-node variant wants the transpose (bQ = 1), via a 32x32 smem tile.
+__global__ void __launch_bounds__(256) sm100_dbias_reduce_kernel(const float* __restrict__ planes, float* __restrict__ dBias,
+                                                                 int BH, int N, int G, int transpose) {
+    __shared__ float tile[32][33];
+    const int bh = blockIdx.z, q0 = blockIdx.y * 32, k0 = blockIdx.x * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const long long pstride = (long long)BH * N * N;
+    for (int j = ty; j < 32; j += 8) {
+        const long long o = (long long)bh * N * N + (long long)(q0 + j) * N + k0 + tx;
+        float acc = planes[o];
+        for (int g = 1; g < G; ++g) acc += planes[o + g * pstride];
+        if (transpose) tile[j][tx] = acc; else dBias[o] = acc;
+    }
+    if (transpose) {
+        __syncthreads();
+        for (int j = ty; j < 32; j += 8) dBias[(long long)bh * N * N + (long long)(k0 + j) * N + q0 + tx] = tile[tx][j];
+    }
 }
 
 }  // namespace
@@ -659,14 +689,32 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
 // ---- host side ------------------------------------------------------------------------------------------------
 namespace {
 struct BwdWs {
-    size_t d_off, da_off, biast_off, total;
+    size_t d_off, da_off, biast_off, planes_off, total;
+    int G;  // row slices of the dBias kernel
 };
+// Split the broadcast-row axis of the tile-stationary dBias kernel over G CTAs per tile when the tile grid alone
+// cannot fill the 148 SMs (1 CTA/SM): pick G in 1..8 minimising waves * rows-per-CTA.
+int dbias_split(const Problem& p) {
+    const long long tiles = (long long)p.B * p.H * (p.N / 128) * (p.N / 128);
+    int best = 1;
+    double best_cost = 1e30;
+    for (int G = 1; G <= 8; ++G) {
+        if (p.N % G) continue;
+        const double waves = (double)((tiles * G + 147) / 148);
+        const double cost = waves * (p.N / G + 24);  // + per-CTA prologue/drain in row units
+        if (cost < best_cost * 0.97) { best_cost = cost; best = G; }
+    }
+    return best;
+}
 BwdWs bwd_ws_layout(const Problem& p) {
     BwdWs w;
     size_t o = 0;
     w.d_off = o; o += align_up((size_t)p.B * p.N * p.H * p.N * sizeof(float), 256);
     w.da_off = o; o += align_up((size_t)p.B * p.N * p.H * p.N * p.d * 2, 256);
     w.biast_off = o; o += align_up((size_t)p.B * p.H * p.N * p.N * 2, 256);
+    w.G = dbias_split(p);
+    w.planes_off = o;
+    if (w.G > 1) o += align_up((size_t)w.G * p.B * p.H * p.N * p.N * sizeof(float), 256);
     w.total = o;
     return w;
 }
@@ -729,12 +777,22 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
                                                                  (__nv_bfloat16*)dQ);
     }
     TRI_LAUNCH_CHECK("sm100_dq_kernel");
+    float* planes = (float*)((char*)ws + w.planes_off);
     {
         ProfScope ps("sm100_dbias_kernel", st);
-        const unsigned grid = (unsigned)((long long)p.B * p.H * (p.N / 128) * (p.N / 128));
-        sm100_dbias_kernel<<<grid, 256, DbiasSmem::total, st>>>(tQ128, tA128, tK128, tV128, tBqk, p, mask, LSE, Dws, dBias);
+        const unsigned grid = (unsigned)((long long)p.B * p.H * (p.N / 128) * (p.N / 128) * w.G);
+        sm100_dbias_kernel<<<grid, 256, DbiasSmem::total, st>>>(tQ128, tA128, tK128, tV128, tBqk, p, mask, LSE, Dws, dBias,
+                                                                planes, w.G);
     }
     TRI_LAUNCH_CHECK("sm100_dbias_kernel");
+    if (w.G > 1) {
+        {
+            ProfScope ps("sm100_dbias_reduce_kernel", st);
+            sm100_dbias_reduce_kernel<<<dim3(p.N / 32, p.N / 32, p.B * p.H), 256, 0, st>>>(
+                planes, dBias, p.B * p.H, p.N, w.G, p.variant == TRI_ENDING ? 1 : 0);
+        }
+        TRI_LAUNCH_CHECK("sm100_dbias_reduce_kernel");
+    }
     return TRI_OK;
 }
 
