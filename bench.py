@@ -181,10 +181,50 @@ def workload_name(cfg) -> str:
 
 
 # ------------------------------------------------------------------------------------------------
+# multi-rank host logic (device-agnostic: tested with the gloo backend on CPU, world_size 2)
+# ------------------------------------------------------------------------------------------------
+def rank_config(cfg, rank: int):
+    """Weak scaling: every rank draws its OWN batch of the workload (rows are independent problems,
+    no data-path collective): same shapes, seed offset by the rank."""
+    return tri_inputs.Config(**{**cfg.__dict__, "seed": cfg.seed + 1000 * rank})
+
+
+def max_over_ranks(ms: float, device, world: int) -> float:
+    """The job's step time is the slowest rank's (all-reduce MAX of the device-measured milliseconds)."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(cfg, world: int, ms_step: float) -> float:
+    """Whole-job model TFLOP/s: all ranks' FLOP over the max-over-ranks step time."""
+    return model_flop(cfg) * world / (ms_step * 1e-3) / 1e12
+
+
+# ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
 # executed tensor FLOP per logit-pass of each kernel, in units of B*H*N^3*d (2 per matmul)
 KERNEL_FLOP_UNITS = (("fwd", 4.0), ("dkdv", 8.0), ("dq", 6.0), ("dbias", 4.0))
+
+
+def ncu_traffic(kernel: str, cfg):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture of this workload
+    (profiles/r1b_traffic_<workload>.json.txt, written from profiles/r1b_sm100_ncu_full_cfg4.md), else None."""
+    path = os.path.join(ROOT, "profiles", f"r1b_traffic_{cfg.name}.json.txt")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        table = json.load(f).get("dram_bytes_per_launch", {})
+    for k, v in table.items():
+        if k == kernel or k.startswith(kernel) or kernel.startswith(k):
+            return v
+    return None
 
 
 def kernel_flop(name: str, cfg) -> float | None:
@@ -214,7 +254,7 @@ def run_ours(args, cfg):
     peaks = load_peaks()
 
     # ---- inputs: seeded synthetic, rounded to bf16 once; each rank draws its own batch (weak scaling)
-    rcfg = tri_inputs.Config(**{**cfg.__dict__, "seed": cfg.seed + 1000 * rank})
+    rcfg = rank_config(cfg, rank)
     x = tri_inputs.make_inputs(rcfg)
     tdt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
     names = ("Q", "K", "V", "G", "bias", "dO")
@@ -261,13 +301,10 @@ def run_ours(args, cfg):
     launches = tri.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     peak_bytes = torch.cuda.max_memory_allocated()
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dev, world)
     ms_step = ms_total / args.steps
     flop_all = model_flop(cfg) * world
-    value = flop_all / (ms_step * 1e-3) / 1e12
+    value = aggregate_value(cfg, world, ms_step)
 
     # ---- e2e: the same step through tri_attn_step_host on pinned HOST buffers (H2D + D2H inside)
     hout = {k: torch.empty_like(host["Q"]).pin_memory() for k in ("O", "dQ", "dK", "dV", "dG")}
@@ -286,10 +323,7 @@ def run_ours(args, cfg):
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1) / e2e_steps
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, dev, world)
     h2d = sum(v.numel() * v.element_size() for v in hin.values() if v is not None)
     d2h = sum(v.numel() * v.element_size() for v in hout.values())
     if world > 1:
@@ -312,7 +346,7 @@ def run_ours(args, cfg):
             # fp32 CUDA-core kernels: 148 SMs x 128 FMA lanes x 2 flop x max SM clock
             peak = 148 * 128 * 2 * 1.965e9 / 1e12
         roof = {"kernel": dom, "bound": bound, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peaks["source"] + (" sustained" if sustained else " burst") if bound == "tensor"
+                "traffic": ncu_traffic(dom, cfg), "peak_source": peaks["source"] + (" sustained" if sustained else " burst") if bound == "tensor"
                 else "derived: 148 SM x 128 lanes x 2 x 1.965 GHz", "flop_per_launch": dflop, "ms_per_launch": dms / dn}
     else:
         U = B * N * H * N * d * (2 if cfg.dtype == "bf16" else 4)
