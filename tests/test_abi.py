@@ -68,7 +68,8 @@ def test_workspace_is_quadratic_not_cubic(lib, variant, dtype):
         for fn in (lib.tri_attn_fwd_workspace_bytes, lib.tri_attn_bwd_workspace_bytes):
             w = fn(B, N, H, d, variant, dtype)
             assert w >= 256
-            assert w <= 64 * B * H * N * N + (1 << 20), (N, w)       # O(N^2 H) with a small constant
+            # O(N^2 H) with a small constant: per (b,h,q,k) element dA 2d = 64 B, D 4 B, bias^T 2 B, <= 8 dBias planes 32 B
+            assert w <= 128 * B * H * N * N + (1 << 20), (N, w)
             assert w < B * H * N * N * N * 2 or N <= 128                # far below the bf16 map
     assert lib.tri_attn_fwd_workspace_bytes(0, 1, 1, 32, 0, 0) == 0
 
