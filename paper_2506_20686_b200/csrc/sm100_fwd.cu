@@ -20,6 +20,7 @@ namespace {
 
 constexpr int BQ = 128, BK = 128, DH = 32;
 constexpr int TILE_BYTES = BQ * DH * 2;  // 8 KB: one 128 x 32 bf16 tile
+constexpr float kLazy = 5.0f;            // lazy-rescale threshold on the running max (natural-log units)
 
 template <int R_>
 struct FwdSmem {
@@ -113,6 +114,7 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
     constexpr uint32_t idescS = make_idesc(128, 128, false, false);
     constexpr uint32_t idescO = make_idesc(128, DH, false, true);
     const float scale = rsqrtf((float)DH);
+    const uint64_t scale2 = pack2(scale, scale);
     float m_run[R_], l_run[R_];
 #pragma unroll
     for (int r = 0; r < R_; ++r) { m_run[r] = -INFINITY; l_run[r] = 0.0f; }
@@ -159,8 +161,8 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
                         const int col = c32 * 32 + j * 8 + e * 2;
-                        x[col] = fmaf(__uint_as_float(raw[j * 8 + e * 2]), scale, bf16_lo(w[e]));
-                        x[col + 1] = fmaf(__uint_as_float(raw[j * 8 + e * 2 + 1]), scale, bf16_hi(w[e]));
+                        unpack2(fma2(pack2(__uint_as_float(raw[j * 8 + e * 2]), __uint_as_float(raw[j * 8 + e * 2 + 1])), scale2,
+                                     pack2(bf16_lo(w[e]), bf16_hi(w[e]))), x[col], x[col + 1]);
                     }
                 }
             }
@@ -176,27 +178,35 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
             for (int c = 0; c < BK; ++c) mx = fmaxf(mx, x[c]);
 
             // ---- online softmax with the -inf guard of reading A6 ---------------------------------
+            // The running reference m moves only when this tile's maximum exceeds it by more than kLazy (O and l
+            // share the reference, so the result is exact either way): keeps the O rescale out of almost every tile.
             const float m_old = m_run[r];
-            const float m_new = fmaxf(m_old, mx);
+            const bool bump = mx > m_old + kLazy;
+            const float m_new = bump ? mx : m_old;
             const float m_safe = (m_new == -INFINITY) ? 0.0f : m_new;
-            const float alpha = ex2((m_old - m_safe) * kLog2e);
+            const float alpha = bump ? ex2((m_old - m_safe) * kLog2e) : 1.0f;
             const float mneg = -m_safe * kLog2e;
-            float lsum = 0.0f;
+            const uint64_t l2e2 = pack2(kLog2e, kLog2e), mneg2 = pack2(mneg, mneg);
+            uint64_t lacc = pack2(0.0f, 0.0f);
 #pragma unroll
             for (int c16 = 0; c16 < BK / 32; ++c16) {  // 32 keys -> 16 packed columns per store
                 uint32_t pk[16];
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
-                    const float p0 = ex2(fmaf(x[c16 * 32 + 2 * e], kLog2e, mneg));
-                    const float p1 = ex2(fmaf(x[c16 * 32 + 2 * e + 1], kLog2e, mneg));
-                    lsum += p0 + p1;
+                    float a0, a1;
+                    unpack2(fma2(pack2(x[c16 * 32 + 2 * e], x[c16 * 32 + 2 * e + 1]), l2e2, mneg2), a0, a1);
+                    const float p0 = ex2(a0), p1 = ex2(a1);
+                    lacc = add2(lacc, pack2(p0, p1));
                     pk[e] = pack_bf16(p0, p1);
                 }
                 tmem_st16(tS + lane_off + c16 * 16, pk);
             }
+            float l0, l1;
+            unpack2(lacc, l0, l1);
+            const float lsum = l0 + l1;
             l_run[r] = l_run[r] * alpha + lsum;
             m_run[r] = m_new;
-            if (kb > 0 && __any_sync(0xffffffffu, m_new > m_old)) {  // rescale the accumulator O_r
+            if (kb > 0 && __any_sync(0xffffffffu, bump)) {  // rescale the accumulator O_r
                 uint32_t o[32];
                 tmem_ld32(tmem + lane_off + 128 + r * 32, o);
                 tmem_ld_wait();
@@ -317,9 +327,11 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK) ||
         !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane(&tB, bias_qk, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
-    static const bool v1 = getenv("TRI_FWD_V1") != nullptr;
-    if (v1) return launch_fwd<4>(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
-    return sm100_fwd2_launch(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
+    // Default: this file's kernel (2 CTAs/SM, 1.95 ms at cfg4).  TRI_FWD_WS=1 selects the warp-specialised two-slot
+    // kernel of sm100_fwd2.cu (2.20 ms at cfg4; kept for A/B and as the base of the next round's pipelining work).
+    static const bool ws_kernel = getenv("TRI_FWD_WS") != nullptr;
+    if (ws_kernel) return sm100_fwd2_launch(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
+    return launch_fwd<4>(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
 }
 
 }  // namespace tri
