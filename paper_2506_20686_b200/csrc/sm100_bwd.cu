@@ -63,7 +63,7 @@ struct DkdvSmem {
     static constexpr int kv_off = 0;                          // R_ x (K, V) 128x32
     static constexpr int qa_off = kv_off + R_ * 2 * T128;     // 2 stages x (Q, dA) 64x32
     static constexpr int bias_off = qa_off + 2 * 2 * T64;     // [128 k][64 q] bf16, SWIZZLE_128B
-    static constexpr int ld_off = bias_off + 16384;           // 2 stages x (nl[64], D[64]) floats
+    static constexpr int ld_off = bias_off + 2 * 16384;       // (bias double buffered) ; 2 stages x (nl[64], D[64]) floats
     static constexpr int bar_off = ld_off + 2 * 128 * 4;
     static constexpr int total = bar_off + 64 + 1024;
 };
@@ -88,9 +88,9 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
     uint64_t* bars = (uint64_t*)(smem + L::bar_off);
     uint64_t* bar_kv = bars + 0;
     uint64_t* bar_qa = bars + 1;  // [2]
-    uint64_t* bar_bias = bars + 3;
+    uint64_t* bar_bias = bars + 5;  // [2]
     uint64_t* bar_mma = bars + 4;
-    uint32_t* tmem_slot = (uint32_t*)(bars + 5);
+    uint32_t* tmem_slot = (uint32_t*)(bars + 7);
 
     // 256 threads: a key row (TMEM lane) is shared by two threads, warps w and w+4, 32 query columns each
     const int tid = threadIdx.x, warp = tid >> 5, chalf = warp >> 2;
@@ -105,7 +105,8 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
 
     if (tid == 0) {
         prefetch_tmap(&tmQ64); prefetch_tmap(&tmA64); prefetch_tmap(&tmK128); prefetch_tmap(&tmV128); prefetch_tmap(&tmBiasKQ);
-        mbar_init(bar_kv, 1); mbar_init(bar_qa, 1); mbar_init(bar_qa + 1, 1); mbar_init(bar_bias, 1); mbar_init(bar_mma, 1);
+        mbar_init(bar_kv, 1); mbar_init(bar_qa, 1); mbar_init(bar_qa + 1, 1); mbar_init(bar_bias, 1); mbar_init(bar_bias + 1, 1);
+        mbar_init(bar_mma, 1);
         fence_barrier_init();
     }
     if (warp == 0) tmem_alloc<TCOLS>(tmem_slot);
@@ -132,6 +133,10 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
         load_qa(0);
         mbar_expect_tx(bar_bias, 16384);
         tma_load_3d(sBias, &tmBiasKQ, bar_bias, 0, k0, bh);
+        if (NQT > 1) {
+            mbar_expect_tx(bar_bias + 1, 16384);
+            tma_load_3d(sBias + 16384, &tmBiasKQ, bar_bias + 1, 64, k0, bh);
+        }
     }
     // per-tile LSE / D of the 64 query columns: threads 0..63 fetch LSE, 64..127 fetch D
     auto ld_val = [&](int t) -> float {
@@ -178,7 +183,8 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
             mbar_wait(bar_mma, t & 1);
             tc_fence_after();
             if (tid == 0 && t + 1 < T) load_qa(t + 1);
-            if (r == 0) mbar_wait(bar_bias, qt & 1);
+            if (r == 0) mbar_wait(bar_bias + (qt & 1), (qt >> 1) & 1);
+            const uint8_t* sB = sBias + (qt & 1) * 16384;
             const float* nlq = sLD + st * 128;
             const float* ddq = nlq + 64;
             {
@@ -188,7 +194,7 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
                 tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
                 uint4 bv[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sBias + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
+                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sB + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
                 tmem_ld_wait();
                 uint32_t pp[16], ds[16];
                 if (keep[r]) {
@@ -235,9 +241,9 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
 #pragma unroll
                 for (int ks = 0; ks < 4; ++ks)
                     mma_ts(tdK, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dq + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
-                if (r == R_ - 1 && qt + 1 < NQT) {
-                    mbar_expect_tx(bar_bias, 16384);
-                    tma_load_3d(sBias, &tmBiasKQ, bar_bias, (qt + 1) * 64, k0, bh);
+                if (r == R_ - 1 && qt + 2 < NQT) {  // every thread is past its reads of buffer qt&1: refill it with qt+2
+                    mbar_expect_tx(bar_bias + (qt & 1), 16384);
+                    tma_load_3d(sBias + (qt & 1) * 16384, &tmBiasKQ, bar_bias + (qt & 1), (qt + 2) * 64, k0, bh);
                 }
             }
         }
