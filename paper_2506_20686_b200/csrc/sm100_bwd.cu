@@ -8,6 +8,8 @@
 //   dbias    tile-stationary: one CTA owns a 128x128 tile of dBias in registers and streams over ALL broadcast
 //            rows in ascending order (S, dP double-buffered in TMEM) -- deterministic, replaces the paper's
 //            tl.atomic_add; workspace stays O(N^2 H d).
+#include <stdlib.h>
+
 #include "sm100_common.cuh"
 #include "tri_common.cuh"
 
@@ -164,7 +166,7 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
 #pragma unroll
         for (int r = 0; r < R_; ++r) {
             const int t = qt * R_ + r, st = t & 1;
-            if (tid == 0) {
+            if (warp == 0) {  // warp-uniform so the descriptors stay in uniform registers; one elected lane issues
                 if (t == 0) mbar_wait(bar_kv, 0);
                 mbar_wait(bar_qa + st, (t >> 1) & 1);
                 tc_fence_after();
@@ -172,11 +174,14 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
                 const uint64_t dv = make_desc_sw64(smem_u32(sKV + r * 2 * T128 + T128));
                 const uint64_t dq = make_desc_sw64(smem_u32(sQA + st * 2 * T64));
                 const uint64_t da = make_desc_sw64(smem_u32(sQA + st * 2 * T64 + T64));
-                mma_ss(tS, dk, dq, idescS, 0);
-                mma_ss(tS, dk + 2, dq + 2, idescS, 1);
-                mma_ss(tDP, dv, da, idescS, 0);
-                mma_ss(tDP, dv + 2, da + 2, idescS, 1);
-                mma_commit(bar_mma);
+                if (elect_one()) {
+                    mma_ss(tS, dk, dq, idescS, 0);
+                    mma_ss(tS, dk + 2, dq + 2, idescS, 1);
+                    mma_ss(tDP, dv, da, idescS, 0);
+                    mma_ss(tDP, dv + 2, da + 2, idescS, 1);
+                    mma_commit(bar_mma);
+                }
+                __syncwarp();
             }
             float ldnext = 0.0f;
             if (t + 1 < T && tid < 128) ldnext = ld_val(t + 1);
@@ -230,21 +235,24 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
             tmem_st_wait();
             tc_fence_before();
             __syncthreads();
-            if (tid == 0) {
+            if (warp == 0) {
                 tc_fence_after();
                 const uint64_t dq = make_desc_sw64(smem_u32(sQA + st * 2 * T64));
                 const uint64_t da = make_desc_sw64(smem_u32(sQA + st * 2 * T64 + T64));
                 const uint32_t tdV = tmem + 128 + r * 64, tdK = tdV + 32;
+                if (elect_one()) {
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks)  // A columns: k-steps 0,1 at [0,16), k-steps 2,3 at [32,48)
-                    mma_ts(tdV, tS + (ks >> 1) * 32 + (ks & 1) * 8, da + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
+                    for (int ks = 0; ks < 4; ++ks)  // A columns: k-steps 0,1 at [0,16), k-steps 2,3 at [32,48)
+                        mma_ts(tdV, tS + (ks >> 1) * 32 + (ks & 1) * 8, da + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks)
-                    mma_ts(tdK, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dq + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
-                if (r == R_ - 1 && qt + 2 < NQT) {  // every thread is past its reads of buffer qt&1: refill it with qt+2
-                    mbar_expect_tx(bar_bias + (qt & 1), 16384);
-                    tma_load_3d(sBias + (qt & 1) * 16384, &tmBiasKQ, bar_bias + (qt & 1), (qt + 2) * 64, k0, bh);
+                    for (int ks = 0; ks < 4; ++ks)
+                        mma_ts(tdK, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dq + (uint64_t)ks * 64, idescO, (qt > 0 || ks > 0) ? 1u : 0u);
+                    if (r == R_ - 1 && qt + 2 < NQT) {  // every thread is past its reads of buffer qt&1: refill it with qt+2
+                        mbar_expect_tx(bar_bias + (qt & 1), 16384);
+                        tma_load_3d(sBias + (qt & 1) * 16384, &tmBiasKQ, bar_bias + (qt & 1), (qt + 2) * 64, k0, bh);
+                    }
                 }
+                __syncwarp();
             }
         }
     }
@@ -380,7 +388,7 @@ __global__ void __launch_bounds__(256, 2) sm100_dq_kernel(const __grid_constant_
 #pragma unroll
         for (int r = 0; r < R_; ++r) {
             const int t = kt * R_ + r, st = t & 1;
-            if (tid == 0) {
+            if (warp == 0) {  // warp-uniform so the descriptors stay in uniform registers; one elected lane issues
                 if (t == 0) mbar_wait(bar_qa, 0);
                 mbar_wait(bar_kv + st, (t >> 1) & 1);
                 tc_fence_after();
@@ -388,11 +396,14 @@ __global__ void __launch_bounds__(256, 2) sm100_dq_kernel(const __grid_constant_
                 const uint64_t da = make_desc_sw64(smem_u32(sQA + r * 2 * T128 + T128));
                 const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * T64));
                 const uint64_t dv = make_desc_sw64(smem_u32(sKV + st * 2 * T64 + T64));
-                mma_ss(tS, dq, dk, idescS, 0);
-                mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-                mma_ss(tDP, da, dv, idescS, 0);
-                mma_ss(tDP, da + 2, dv + 2, idescS, 1);
-                mma_commit(bar_mma);
+                if (elect_one()) {
+                    mma_ss(tS, dq, dk, idescS, 0);
+                    mma_ss(tS, dq + 2, dk + 2, idescS, 1);
+                    mma_ss(tDP, da, dv, idescS, 0);
+                    mma_ss(tDP, da + 2, dv + 2, idescS, 1);
+                    mma_commit(bar_mma);
+                }
+                __syncwarp();
             }
             float mnext = 0.0f;
             if (mask && t + 1 < T) mnext = mask_val(t + 1);
@@ -443,17 +454,20 @@ __global__ void __launch_bounds__(256, 2) sm100_dq_kernel(const __grid_constant_
             tmem_st_wait();
             tc_fence_before();
             if (mask) anymask = __syncthreads_or(mnext != 0.0f); else __syncthreads();
-            if (tid == 0) {
+            if (warp == 0) {
                 tc_fence_after();
                 const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * T64));
+                if (elect_one()) {
 #pragma unroll
-                for (int ks = 0; ks < 4; ++ks)
-                    mma_ts(tmem + 128 + r * 32, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dk + (uint64_t)ks * 64, idescO,
-                           (kt > 0 || ks > 0) ? 1u : 0u);
-                if (r == R_ - 1 && kt + 1 < NKT) {
-                    mbar_expect_tx(bar_bias, 16384);
-                    tma_load_3d(sBias, &tmBiasQK, bar_bias, (kt + 1) * 64, q0, bh);
+                    for (int ks = 0; ks < 4; ++ks)
+                        mma_ts(tmem + 128 + r * 32, tDP + (ks >> 1) * 32 + (ks & 1) * 8, dk + (uint64_t)ks * 64, idescO,
+                               (kt > 0 || ks > 0) ? 1u : 0u);
+                    if (r == R_ - 1 && kt + 1 < NKT) {
+                        mbar_expect_tx(bar_bias, 16384);
+                        tma_load_3d(sBias, &tmBiasQK, bar_bias, (kt + 1) * 64, q0, bh);
+                    }
                 }
+                __syncwarp();
             }
         }
     }
@@ -551,7 +565,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         tma_load_5d(base + 3 * T128, &tmV128, bar_full + s, 0, k0, rb + r, h, b);
     };
     constexpr uint32_t idescS = make_idesc(128, 128, false, false);
-    auto issue_mma = [&](int r) {
+    auto issue_mma = [&](int r) {  // called by the whole warp 0 (warp-uniform); one elected lane issues
         const int s = r % NST, j = r & 1;
         mbar_wait(bar_full + s, (r / NST) & 1);
         tc_fence_after();
@@ -559,11 +573,14 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         const uint64_t dq = make_desc_sw64(smem_u32(base)), da = make_desc_sw64(smem_u32(base + T128));
         const uint64_t dk = make_desc_sw64(smem_u32(base + 2 * T128)), dv = make_desc_sw64(smem_u32(base + 3 * T128));
         const uint32_t tS = tmem + j * 256, tDP = tS + 128;
-        mma_ss(tS, dq, dk, idescS, 0);
-        mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-        mma_ss(tDP, da, dv, idescS, 0);
-        mma_ss(tDP, da + 2, dv + 2, idescS, 1);
-        mma_commit(bar_mma + j);
+        if (elect_one()) {
+            mma_ss(tS, dq, dk, idescS, 0);
+            mma_ss(tS, dq + 2, dk + 2, idescS, 1);
+            mma_ss(tDP, da, dv, idescS, 0);
+            mma_ss(tDP, da + 2, dv + 2, idescS, 1);
+            mma_commit(bar_mma + j);
+        }
+        __syncwarp();
     };
     if (tid == 0) {
         for (int r = 0; r < NST && r < NR; ++r) load_ops(r);
@@ -584,7 +601,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         if (tid < 128) sMask[tid] = mv;
         anymask = __syncthreads_or(mv != 0.0f);
     }
-    if (tid == 0) issue_mma(0);
+    if (warp == 0) issue_mma(0);
     float lse_n = __ldg(LSE + lse_off(0)), dd_n = __ldg(Dws + lse_off(0));
     const float scale = rsqrtf((float)DH);
     uint64_t acc2[32];  // dBias tile: my 64 columns as fp32 pairs
@@ -595,7 +612,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
 
     for (int r = 0; r < NR; ++r) {
         const int j = r & 1;
-        if (tid == 0 && r + 1 < NR) issue_mma(r + 1);
+        if (warp == 0 && r + 1 < NR) issue_mma(r + 1);
         const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e, dd = dd_n;
         const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd, -dd);
         float mnext = 0.0f;
@@ -776,13 +793,20 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
                                                                        (__nv_bfloat16*)dK, (__nv_bfloat16*)dV);
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
-    {
-        ProfScope ps("sm100_dq_kernel", st);
-        const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
-        sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
-                                                                 (__nv_bfloat16*)dQ);
+    // Default: sm100_dq_kernel (2 CTAs/SM, 1.96 ms at cfg4).  TRI_DQ_WS=1 selects the two-slot software-pipelined kernel of
+    // sm100_dq2.cu (2.37 ms at cfg4), kept for A/B.
+    static const bool dq_ws = getenv("TRI_DQ_WS") != nullptr;
+    if (!dq_ws) {
+        {
+            ProfScope ps("sm100_dq_kernel", st);
+            const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
+            sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
+                                                                     (__nv_bfloat16*)dQ);
+        }
+        TRI_LAUNCH_CHECK("sm100_dq_kernel");
+    } else {
+        if ((s = sm100_dq2_launch(p, tQ128, tA128, tK64, tV64, tBqk, mask, LSE, Dws, dQ, st)) != TRI_OK) return s;
     }
-    TRI_LAUNCH_CHECK("sm100_dq_kernel");
     float* planes = (float*)((char*)ws + w.planes_off);
     {
         ProfScope ps("sm100_dbias_kernel", st);

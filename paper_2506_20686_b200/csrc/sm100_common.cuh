@@ -37,6 +37,17 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+__device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {  // non-blocking probe
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {
     }
@@ -69,6 +80,13 @@ __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.b
 __device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 // generic-proxy smem writes -> visible to the async proxy (TMA store / UMMA operand reads)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// One lane of a fully converged warp (warp-uniform control flow keeps descriptor arithmetic in uniform registers)
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 
 // ---- tcgen05: TMEM allocation --------------------------------------------------------------------
 template <int COLS>
@@ -236,6 +254,9 @@ bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d,
 bool make_tmap_plane(CUtensorMap* out, const void* base, int BH, int N, int box_rows);
 
 struct Problem;
+tri_status sm100_dq2_launch(const Problem& p, const CUtensorMap& tQ128, const CUtensorMap& tA128, const CUtensorMap& tK64,
+                            const CUtensorMap& tV64, const CUtensorMap& tBqk, const unsigned char* mask, const float* LSE,
+                            const float* Dws, void* dQ, cudaStream_t st);
 tri_status sm100_fwd2_launch(const Problem& p, const CUtensorMap& tQ, const CUtensorMap& tK, const CUtensorMap& tV,
                              const CUtensorMap& tB, const void* G, const unsigned char* mask, void* O, float* LSE,
                              cudaStream_t st);

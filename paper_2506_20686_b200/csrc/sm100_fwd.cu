@@ -123,15 +123,18 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
 #pragma unroll
         for (int r = 0; r < R_; ++r) {
             const int t = kb * R_ + r, st = t & 1;
-            if (tid == 0) {
+            if (warp == 0) {  // warp-uniform so the descriptors stay in uniform registers; one elected lane issues
                 if (t == 0) mbar_wait(bar_q, 0);
                 mbar_wait(bar_kv + st, (t >> 1) & 1);
                 tc_fence_after();
                 const uint64_t dq = make_desc_sw64(smem_u32(sQ + r * TILE_BYTES));
                 const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * TILE_BYTES));
-                mma_ss(tS, dq, dk, idescS, 0);
-                mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-                mma_commit(bar_mma);
+                if (elect_one()) {
+                    mma_ss(tS, dq, dk, idescS, 0);
+                    mma_ss(tS, dq + 2, dk + 2, idescS, 1);
+                    mma_commit(bar_mma);
+                }
+                __syncwarp();
             }
             float mnext = 0.0f;
             if (mask && t + 1 < T) mnext = mask_val(t + 1);
@@ -218,13 +221,16 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
             tmem_st_wait();
             tc_fence_before();
             if (mask) anymask = __syncthreads_or(mnext != 0.0f); else __syncthreads();
-            if (tid == 0) {
+            if (warp == 0) {
                 tc_fence_after();
                 const uint64_t dv = make_desc_sw64(smem_u32(sKV + st * 2 * TILE_BYTES + TILE_BYTES));
+                if (elect_one()) {
 #pragma unroll
-                for (int ks = 0; ks < BK / 16; ++ks)
-                    mma_ts(tmem + 128 + r * 32, tS + ks * 8, dv + (uint64_t)ks * 64, idescO, (kb > 0 || ks > 0) ? 1u : 0u);
-                if (r == R_ - 1 && kb + 1 < NKB) load_bias(kb + 1);  // every thread is past its bias reads
+                    for (int ks = 0; ks < BK / 16; ++ks)
+                        mma_ts(tmem + 128 + r * 32, tS + ks * 8, dv + (uint64_t)ks * 64, idescO, (kb > 0 || ks > 0) ? 1u : 0u);
+                    if (r == R_ - 1 && kb + 1 < NKB) load_bias(kb + 1);  // every thread is past its bias reads
+                }
+                __syncwarp();
             }
         }
     }
