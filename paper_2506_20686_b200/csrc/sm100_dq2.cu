@@ -15,13 +15,6 @@
 namespace tri {
 using namespace sm100;
 
-#ifdef TRI_TIMING
-__device__ long long g_tri_timing_dq[64 * 8];
-#define TRI_TS(i) do { } while (0)
-#else
-#define TRI_TS(i) do { } while (0)
-#endif
-
 namespace {
 
 constexpr int DH = 32;
@@ -104,22 +97,14 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
     };
     constexpr uint32_t idescS = make_idesc(128, 64, false, false);
     constexpr uint32_t idescO = make_idesc(128, DH, false, true);
-#ifdef TRI_TIMING
-#define TRI_TI(i) do { if (blockIdx.x == 7 && tid == 0 && t < 64) g_tri_timing_dq[t * 8 + (i)] = clock64(); } while (0)
-#else
-#define TRI_TI(i) do { } while (0)
-#endif
     auto issue_ss = [&](int t) {  // S, dP of tile t: called by the whole first warp of the slot (warp-uniform)
         const int r = t % RS, st = t % NST;
-        TRI_TI(0);
         mbar_wait(bar_kv + st, (t / NST) & 1);
-        TRI_TI(1);
         tc_fence_after();
         const uint64_t dq = make_desc_sw64(smem_u32(sQA + (slot * RS + r) * 2 * T128));
         const uint64_t da = make_desc_sw64(smem_u32(sQA + (slot * RS + r) * 2 * T128 + T128));
         const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * T64));
         const uint64_t dv = make_desc_sw64(smem_u32(sKV + st * 2 * T64 + T64));
-        TRI_TI(2);
         if (elect_one()) {
             mma_ss(tS, dq, dk, idescS, 0);
             mma_ss(tS, dq + 2, dk + 2, idescS, 1);
@@ -128,7 +113,6 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
             mma_commit(bar_mma);
         }
         __syncwarp();
-        TRI_TI(6);
     };
 
     if (stid == 0) {
@@ -176,10 +160,8 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
             const int t = kt * RS + r, st = t % NST;
             float mnext = 0.0f;
             if (mask && t + 1 < T) mnext = mask_val(t + 1);
-            TRI_TS(0);
             mbar_wait(bar_mma, t & 1);  // S(t), dP(t) ready
             tc_fence_after();
-            TRI_TS(1);
             if (r == 0) mbar_wait(bars + D_BIAS_FULL + (kt & 1), (kt >> 1) & 1);
             uint32_t sraw[32], dpraw[32];
             tmem_ld32(tS + lane_off + chalf * 32, sraw);
@@ -190,11 +172,8 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
             for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sB + row * 128 + (((chalf * 4 + j) ^ (row & 7)) << 4));
             tmem_ld_wait();
             tc_fence_before();
-            TRI_TS(2);
             named_bar_sync(bar_id, 256);  // [A] the whole tile is in registers: S / dP may be overwritten
-            TRI_TS(3);
             if (swarp == 0 && t + 1 < T) issue_ss(t + 1);
-            TRI_TS(4);
 
             if (anymask) {
                 const float* mrow = sMask + (t & 1) * 64 + chalf * 32;
@@ -224,7 +203,6 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
                     ds[j * 4 + e] = pack_bf16(s0, s1);
                 }
             }
-            TRI_TS(5);
             if (t >= 1) {  // dQ MMAs of tile t-1 done: dS buffer free, K/V ring slot (t-1)%NST free
                 mbar_wait(bar_ts, (t - 1) & 1);
                 tc_fence_after();
@@ -234,9 +212,7 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
             if (mask && t + 1 < T && stid < 64) sMask[((t + 1) & 1) * 64 + stid] = mnext;
             tmem_st_wait();
             tc_fence_before();
-            TRI_TS(6);
             if (mask) anymask = named_bar_or(bar_id, 256, mnext != 0.0f); else named_bar_sync(bar_id, 256);  // [B]
-            TRI_TS(7);
             if (swarp == 0) {  // warp-uniform: the elected lane issues dQ_r += dS K
                 tc_fence_after();
                 const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * T64));
@@ -299,11 +275,5 @@ tri_status sm100_dq2_launch(const Problem& p, const CUtensorMap& tQ128, const CU
     TRI_LAUNCH_CHECK("sm100_dq2_kernel");
     return TRI_OK;
 }
-
-#ifdef TRI_TIMING
-extern "C" __attribute__((visibility("default"))) int tri_debug_timing_dq(long long* out) {
-    return (int)cudaMemcpyFromSymbol(out, g_tri_timing_dq, sizeof(long long) * 64 * 8);
-}
-#endif
 
 }  // namespace tri
