@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
             if (t + 1 < T && tid < 128) ldnext = ld_val(t + 1);
             mbar_wait(bar_mma, t & 1);
             tc_fence_after();
-            if (tid == 0 && t + 1 < T) load_qa(t + 1);
+            if (tid == 32 && t + 1 < T) load_qa(t + 1);  // warp 1 issues the TMA loads, warp 0 the MMAs
             if (r == 0) mbar_wait(bar_bias + (qt & 1), (qt >> 1) & 1);
             const uint8_t* sB = sBias + (qt & 1) * 16384;
             const float* nlq = sLD + st * 128;
@@ -409,7 +409,7 @@ __global__ void __launch_bounds__(256, 2) sm100_dq_kernel(const __grid_constant_
             if (mask && t + 1 < T) mnext = mask_val(t + 1);
             mbar_wait(bar_mma, t & 1);
             tc_fence_after();
-            if (tid == 0 && t + 1 < T) load_kv(t + 1);
+            if (tid == 32 && t + 1 < T) load_kv(t + 1);  // warp 1 issues the TMA loads, warp 0 the MMAs
             if (r == 0) mbar_wait(bar_bias, kt & 1);
             const float* mrow = sMask + st * 64;
             {
@@ -623,7 +623,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
         }
         mbar_wait(bar_mma + j, (r >> 1) & 1);
         tc_fence_after();
-        if (tid == 0 && r + NST < NR) load_ops(r + NST);
+        if (tid == 128 && r + NST < NR) load_ops(r + NST);  // warp 4 issues the TMA loads, warp 0 the MMAs
         const uint32_t tS = tmem + j * 256 + half * 64, tDP = tS + 128;
         const float* mrow = sMask + j * 128 + half * 64;
 #pragma unroll

@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
             if (mask && t + 1 < T) mnext = mask_val(t + 1);
             mbar_wait(bar_mma, t & 1);
             tc_fence_after();
-            if (tid == 0 && t + 1 < T) load_kv(t + 1);  // stage (t+1)&1 was last read by tile t-1: complete
+            if (tid == 32 && t + 1 < T) load_kv(t + 1);  // (warp 1: warp 0 carries the MMA issue) stage (t+1)&1 was last read by tile t-1
             if (r == 0) mbar_wait(bar_bias, kb & 1);
 
             // ---- scores of my query row: x = scale*S + bias (+ mask) ---------------------------------------
