@@ -504,11 +504,11 @@ struct DbiasSmem {
     static constexpr int op_off = 0;                         // NST stages x (Q, dA, K, V) 128x32
     static constexpr int bias_off = op_off + NST * 4 * T128; // 2 x [128 q][64 k] bf16, SWIZZLE_128B
     static constexpr int mask_off = bias_off + 32768;        // 2 x 128 floats
-    static constexpr int bar_off = mask_off + 2 * 128 * 4;
-    static constexpr int total = bar_off + 64 + 1024;
+    static constexpr int bar_off = mask_off + 2 * 128 * 4 + 16;  // + two any-flags
+    static constexpr int total = bar_off + 128 + 1024;
 };
 
-__global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant__ CUtensorMap tmQ128,
+__global__ void __launch_bounds__(288, 1) sm100_dbias_kernel(const __grid_constant__ CUtensorMap tmQ128,
                                                           const __grid_constant__ CUtensorMap tmA128,
                                                           const __grid_constant__ CUtensorMap tmK128,
                                                           const __grid_constant__ CUtensorMap tmV128,
@@ -522,15 +522,18 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* sOp = smem + L::op_off;
     uint8_t* sBias = smem + L::bias_off;
-    float* sMask = (float*)(smem + L::mask_off);
+    float* sMask = (float*)(smem + L::mask_off);  // [2][128] floats, then [2] any-flags
+    int* sAny = (int*)(sMask + 256);
     uint64_t* bars = (uint64_t*)(smem + L::bar_off);
-    uint64_t* bar_full = bars + 0;  // [3]
-    uint64_t* bar_mma = bars + 3;   // [2]
+    uint64_t* bar_full = bars + 0;  // [3] TMA ring
+    uint64_t* bar_mma = bars + 3;   // [2] S, dP of a row ready
     uint64_t* bar_bias = bars + 5;
-    uint32_t* tmem_slot = (uint32_t*)(bars + 6);
+    uint64_t* bar_cons = bars + 6;  // [2] all 8 compute warps have S, dP of the row in registers (buffer free)
+    uint32_t* tmem_slot = (uint32_t*)(bars + 8);
 
+    // warps 0-7: compute (TMEM lane quarter = warp & 3, key-column half = warp >> 2); warp 8: TMA + MMA issue + mask staging
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int half = warp >> 2, qrow = (warp & 3) * 32 + lane;
+    const int half = (warp >> 2) & 1, qrow = (warp & 3) * 32 + lane;
     const int NT = p.N / 128;
     int idx = blockIdx.x;
     const int kt = idx % NT; idx /= NT;
@@ -545,7 +548,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
 
     if (tid == 0) {
         prefetch_tmap(&tmQ128); prefetch_tmap(&tmA128); prefetch_tmap(&tmK128); prefetch_tmap(&tmV128); prefetch_tmap(&tmBiasQK);
-        for (int i = 0; i < 6; ++i) mbar_init(bars + i, 1);
+        for (int i = 0; i < 8; ++i) mbar_init(bars + i, (i >= 6) ? 8 : 1);
         fence_barrier_init();
     }
     if (warp == 0) tmem_alloc<512>(tmem_slot);
@@ -554,116 +557,129 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-
-    auto load_ops = [&](int r) {
-        const int s = r % NST;
-        uint8_t* base = sOp + s * 4 * T128;
-        mbar_expect_tx(bar_full + s, 4 * T128);
-        tma_load_5d(base, &tmQ128, bar_full + s, 0, q0, rb + r, h, b);
-        tma_load_5d(base + T128, &tmA128, bar_full + s, 0, q0, rb + r, h, b);
-        tma_load_5d(base + 2 * T128, &tmK128, bar_full + s, 0, k0, rb + r, h, b);
-        tma_load_5d(base + 3 * T128, &tmV128, bar_full + s, 0, k0, rb + r, h, b);
-    };
-    constexpr uint32_t idescS = make_idesc(128, 128, false, false);
-    auto issue_mma = [&](int r) {  // called by the whole warp 0 (warp-uniform); one elected lane issues
-        const int s = r % NST, j = r & 1;
-        mbar_wait(bar_full + s, (r / NST) & 1);
-        tc_fence_after();
-        uint8_t* base = sOp + s * 4 * T128;
-        const uint64_t dq = make_desc_sw64(smem_u32(base)), da = make_desc_sw64(smem_u32(base + T128));
-        const uint64_t dk = make_desc_sw64(smem_u32(base + 2 * T128)), dv = make_desc_sw64(smem_u32(base + 3 * T128));
-        const uint32_t tS = tmem + j * 256, tDP = tS + 128;
-        if (elect_one()) {
-            mma_ss(tS, dq, dk, idescS, 0);
-            mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-            mma_ss(tDP, da, dv, idescS, 0);
-            mma_ss(tDP, da + 2, dv + 2, idescS, 1);
-            mma_commit(bar_mma + j);
-        }
-        __syncwarp();
-    };
-    if (tid == 0) {
-        for (int r = 0; r < NST && r < NR; ++r) load_ops(r);
-        mbar_expect_tx(bar_bias, 32768);
-        tma_load_3d(sBias, &tmBiasQK, bar_bias, k0, q0, bh);
-        tma_load_3d(sBias + 16384, &tmBiasQK, bar_bias, k0 + 64, q0, bh);
-    }
-    auto mask_val = [&](int r) -> float {
-        const unsigned char mk = mask[(long long)b * N * N + (long long)(rb + r) * p.mR + (long long)(k0 + (tid & 127)) * p.mK];
-        return mk ? 0.0f : -INFINITY;
-    };
-    auto lse_off = [&](int r) -> long long {
-        return (long long)b * N * p.H * N + (long long)h * N + (long long)(rb + r) * p.lR + (long long)(q0 + qrow) * p.lQ;
-    };
-    int anymask = 0;
-    if (mask) {
-        const float mv = mask_val(0);
-        if (tid < 128) sMask[tid] = mv;
-        anymask = __syncthreads_or(mv != 0.0f);
-    }
-    if (warp == 0) issue_mma(0);
-    float lse_n = __ldg(LSE + lse_off(0)), dd_n = __ldg(Dws + lse_off(0));
     const float scale = rsqrtf((float)DH);
     uint64_t acc2[32];  // dBias tile: my 64 columns as fp32 pairs
 #pragma unroll
     for (int c = 0; c < 32; ++c) acc2[c] = pack2(0.0f, 0.0f);
-    const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
-    mbar_wait(bar_bias, 0);
 
-    for (int r = 0; r < NR; ++r) {
-        const int j = r & 1;
-        if (warp == 0 && r + 1 < NR) issue_mma(r + 1);
-        const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e, dd = dd_n;
-        const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd, -dd);
-        float mnext = 0.0f;
-        if (r + 1 < NR) {
-            lse_n = __ldg(LSE + lse_off(r + 1));
-            dd_n = __ldg(Dws + lse_off(r + 1));
-            if (mask) mnext = mask_val(r + 1);
+    if (warp == 8) {
+        // =========================== issuer warp (warp-uniform; one elected lane issues TMA / MMA) ===========================
+        auto load_ops = [&](int r) {
+            const int s = r % NST;
+            uint8_t* base = sOp + s * 4 * T128;
+            mbar_expect_tx(bar_full + s, 4 * T128);
+            tma_load_5d(base, &tmQ128, bar_full + s, 0, q0, rb + r, h, b);
+            tma_load_5d(base + T128, &tmA128, bar_full + s, 0, q0, rb + r, h, b);
+            tma_load_5d(base + 2 * T128, &tmK128, bar_full + s, 0, k0, rb + r, h, b);
+            tma_load_5d(base + 3 * T128, &tmV128, bar_full + s, 0, k0, rb + r, h, b);
+        };
+        constexpr uint32_t idescS = make_idesc(128, 128, false, false);
+        if (elect_one()) {
+            for (int r = 0; r < NST && r < NR; ++r) load_ops(r);
+            mbar_expect_tx(bar_bias, 32768);
+            tma_load_3d(sBias, &tmBiasQK, bar_bias, k0, q0, bh);
+            tma_load_3d(sBias + 16384, &tmBiasQK, bar_bias, k0 + 64, q0, bh);
         }
-        mbar_wait(bar_mma + j, (r >> 1) & 1);
-        tc_fence_after();
-        if (tid == 128 && r + NST < NR) load_ops(r + NST);  // warp 4 issues the TMA loads, warp 0 the MMAs
-        const uint32_t tS = tmem + j * 256 + half * 64, tDP = tS + 128;
-        const float* mrow = sMask + j * 128 + half * 64;
+        __syncwarp();
+        for (int r = 0; r < NR; ++r) {
+            const int s = r % NST, j = r & 1;
+            if (r >= 2) mbar_wait(bar_cons + j, ((r - 2) >> 1) & 1);  // row r-2 left TMEM buffer j (and mask slot j)
+            if (mask) {  // keep flags of the 128 keys of this tile in row rb+r -> additive 0 / -inf, plus an any-flag
+                int any = 0;
 #pragma unroll
-        for (int c32 = 0; c32 < 2; ++c32) {
-            uint32_t sraw[32], dpraw[32];
-            tmem_ld32(tS + lane_off + c32 * 32, sraw);
-            tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
-            uint4 bv[4];
+                for (int i = 0; i < 4; ++i) {
+                    const int k = lane * 4 + i;
+                    const unsigned char mk = mask[(long long)b * N * N + (long long)(rb + r) * p.mR + (long long)(k0 + k) * p.mK];
+                    sMask[j * 128 + k] = mk ? 0.0f : -INFINITY;
+                    any |= !mk;
+                }
+                any = __any_sync(0xffffffffu, any);
+                if (lane == 0) sAny[j] = any;
+                __syncwarp();
+            }
+            mbar_wait(bar_full + s, (r / NST) & 1);
+            tc_fence_after();
+            uint8_t* base = sOp + s * 4 * T128;
+            const uint64_t dq = make_desc_sw64(smem_u32(base)), da = make_desc_sw64(smem_u32(base + T128));
+            const uint64_t dk = make_desc_sw64(smem_u32(base + 2 * T128)), dv = make_desc_sw64(smem_u32(base + 3 * T128));
+            const uint32_t tS = tmem + j * 256, tDP = tS + 128;
+            if (elect_one()) {
+                mma_ss(tS, dq, dk, idescS, 0);
+                mma_ss(tS, dq + 2, dk + 2, idescS, 1);
+                mma_ss(tDP, da, dv, idescS, 0);
+                mma_ss(tDP, da + 2, dv + 2, idescS, 1);
+                mma_commit(bar_mma + j);
+            }
+            __syncwarp();
+            if (r >= 1 && r - 1 + NST < NR) {  // MMAs of row r-1 done -> its ring slot is free
+                mbar_wait(bar_mma + ((r - 1) & 1), ((r - 1) >> 1) & 1);
+                if (elect_one()) load_ops(r - 1 + NST);
+                __syncwarp();
+            }
+        }
+    } else {
+        // =========================== compute warps ===========================
+        auto lse_off = [&](int r) -> long long {
+            return (long long)b * N * p.H * N + (long long)h * N + (long long)(rb + r) * p.lR + (long long)(q0 + qrow) * p.lQ;
+        };
+        float lse_n = __ldg(LSE + lse_off(0)), dd_n = __ldg(Dws + lse_off(0));
+        const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
+        mbar_wait(bar_bias, 0);
+        for (int r = 0; r < NR; ++r) {
+            const int j = r & 1;
+            const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e, dd = dd_n;
+            const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd, -dd);
+            if (r + 1 < NR) {
+                lse_n = __ldg(LSE + lse_off(r + 1));
+                dd_n = __ldg(Dws + lse_off(r + 1));
+            }
+            mbar_wait(bar_mma + j, (r >> 1) & 1);
+            tc_fence_after();
+            const int anymask = mask ? sAny[j] : 0;
+            const uint32_t tS = tmem + j * 256 + half * 64, tDP = tS + 128;
+            const float* mrow = sMask + j * 128 + half * 64;
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj)
-                bv[jj] = *(const uint4*)(sBias + half * 16384 + qrow * 128 + (((c32 * 4 + jj) ^ (qrow & 7)) << 4));
-            tmem_ld_wait();
-            if (anymask) {
+            for (int c32 = 0; c32 < 2; ++c32) {
+                uint32_t sraw[32], dpraw[32];
+                tmem_ld32(tS + lane_off + c32 * 32, sraw);
+                tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
+                uint4 bv[4];
 #pragma unroll
-                for (int c4 = 0; c4 < 8; ++c4) {
-                    const float4 mv = *(const float4*)(mrow + c32 * 32 + c4 * 4);
-                    sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);
-                    sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
-                    sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);
-                    sraw[c4 * 4 + 3] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 3]) + mv.w);
+                for (int jj = 0; jj < 4; ++jj)
+                    bv[jj] = *(const uint4*)(sBias + half * 16384 + qrow * 128 + (((c32 * 4 + jj) ^ (qrow & 7)) << 4));
+                tmem_ld_wait();
+                if (anymask) {
+#pragma unroll
+                    for (int c4 = 0; c4 < 8; ++c4) {
+                        const float4 mv = *(const float4*)(mrow + c32 * 32 + c4 * 4);
+                        sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);
+                        sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
+                        sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);
+                        sraw[c4 * 4 + 3] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 3]) + mv.w);
+                    }
+                }
+                if (c32 == 1) {  // my last read of TMEM buffer j and of mask slot j: hand the buffer back to the issuer
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar_cons + j);
+                }
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    const uint32_t w[4] = {bv[jj].x, bv[jj].y, bv[jj].z, bv[jj].w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int c = jj * 8 + e * 2, k2 = (c32 * 32 + c) >> 1;
+                        const uint64_t x2 = fma2(pack2(__uint_as_float(sraw[c]), __uint_as_float(sraw[c + 1])), scale2,
+                                                 pack2(bf16_lo(w[e]), bf16_hi(w[e])));
+                        float a0, a1;
+                        unpack2(fma2(x2, l2e2, nl2), a0, a1);
+                        acc2[k2] = fma2(pack2(ex2(a0), ex2(a1)), add2(pack2(__uint_as_float(dpraw[c]), __uint_as_float(dpraw[c + 1])), nd2), acc2[k2]);
+                    }
                 }
             }
-#pragma unroll
-            for (int jj = 0; jj < 4; ++jj) {
-                const uint32_t w[4] = {bv[jj].x, bv[jj].y, bv[jj].z, bv[jj].w};
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int c = jj * 8 + e * 2, k2 = (c32 * 32 + c) >> 1;
-                    const uint64_t x2 = fma2(pack2(__uint_as_float(sraw[c]), __uint_as_float(sraw[c + 1])), scale2,
-                                             pack2(bf16_lo(w[e]), bf16_hi(w[e])));
-                    float a0, a1;
-                    unpack2(fma2(x2, l2e2, nl2), a0, a1);
-                    acc2[k2] = fma2(pack2(ex2(a0), ex2(a1)), add2(pack2(__uint_as_float(dpraw[c]), __uint_as_float(dpraw[c + 1])), nd2), acc2[k2]);
-                }
-            }
         }
-        if (mask && r + 1 < NR && tid < 128) sMask[(j ^ 1) * 128 + tid] = mnext;
-        tc_fence_before();
-        if (mask) anymask = __syncthreads_or(mnext != 0.0f); else __syncthreads();
     }
+    if (warp < 8) {
     float acc[64];
 #pragma unroll
     for (int c = 0; c < 32; ++c) unpack2(acc2[c], acc[2 * c], acc[2 * c + 1]);
@@ -680,6 +696,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_kernel(const __grid_constant_
 #pragma unroll
             for (int c = 0; c < 64; ++c) out[(long long)c * p.bK] = acc[c];
         }
+    }
     }
     tc_fence_before();
     __syncthreads();
@@ -811,7 +828,7 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     {
         ProfScope ps("sm100_dbias_kernel", st);
         const unsigned grid = (unsigned)((long long)p.B * p.H * (p.N / 128) * (p.N / 128) * w.G);
-        sm100_dbias_kernel<<<grid, 256, DbiasSmem::total, st>>>(tQ128, tA128, tK128, tV128, tBqk, p, mask, LSE, Dws, dBias,
+        sm100_dbias_kernel<<<grid, 288, DbiasSmem::total, st>>>(tQ128, tA128, tK128, tV128, tBqk, p, mask, LSE, Dws, dBias,
                                                                 planes, w.G);
     }
     TRI_LAUNCH_CHECK("sm100_dbias_kernel");
