@@ -191,3 +191,44 @@ def test_step_host_end_to_end_matches_device_path(tri):
     torch.cuda.synchronize()
     for k in pu.OUT_NAMES:
         assert torch.equal(hout[k].view(torch.uint8), dev[k].cpu().view(torch.uint8)), k
+
+
+def test_bitwise_determinism_with_row_split_dbias(tri):
+    """N=384: the dBias kernel splits the broadcast-row axis over 4 CTAs per tile and a second pass adds the
+    partial planes in a fixed order -- the result must still be bitwise reproducible (A16)."""
+    import torch
+
+    cfg = tri_inputs.small_config(1, 384, 2, 32, "bf16", ENDING, 1.0, "random:5", seed=41)
+    x = tri_inputs.make_inputs(cfg)
+    _, a = pu.run_gpu(x, cfg.dtype, cfg.variant)
+    _, b = pu.run_gpu(x, cfg.dtype, cfg.variant)
+    for k in pu.OUT_NAMES:
+        assert torch.equal(a[k].view(torch.uint8), b[k].view(torch.uint8)), k
+
+
+_ALT_SCRIPT = r"""
+import sys, os
+sys.path.insert(0, os.getcwd()); sys.path.insert(0, os.path.join(os.getcwd(), "tests"))
+import oracle, parity_util as pu, tri_inputs
+oracle.build()
+for variant in (0, 1):
+    cfg = tri_inputs.small_config(1, 256, 2, 32, "bf16", variant, 2.0, "tail:9", seed=77)
+    x = tri_inputs.make_inputs(cfg)
+    got, _ = pu.run_gpu(x, "bf16", variant)
+    ref = pu.run_oracle(oracle, x, variant)
+    pu.assert_close(got, ref, pu.TOL["bf16"], what="alt-kernels v%d" % variant)
+print("ALT OK")
+"""
+
+
+def test_alternate_kernels_parity(tri):
+    """The warp-specialised forward (TRI_FWD_WS=1) and the software-pipelined dQ (TRI_DQ_WS=1) are kept for A/B:
+    they must stay parity-green too.  The switches are read once per process, hence the subprocess."""
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, TRI_FWD_WS="1", TRI_DQ_WS="1")
+    r = subprocess.run([sys.executable, "-c", _ALT_SCRIPT], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "ALT OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
