@@ -257,8 +257,7 @@ struct Problem;
 tri_status sm100_dq2_launch(const Problem& p, const CUtensorMap& tQ128, const CUtensorMap& tA128, const CUtensorMap& tK64,
                             const CUtensorMap& tV64, const CUtensorMap& tBqk, const unsigned char* mask, const float* LSE,
                             const float* Dws, void* dQ, cudaStream_t st);
-tri_status sm100_fwd2_launch(const Problem& p, const CUtensorMap& tQ, const CUtensorMap& tK, const CUtensorMap& tV,
+tri_status sm100_fwd3_launch(const Problem& p, const CUtensorMap& tQ, const CUtensorMap& tK, const CUtensorMap& tV,
                              const CUtensorMap& tB, const void* G, const unsigned char* mask, void* O, float* LSE,
                              cudaStream_t st);
-
 }  // namespace tri

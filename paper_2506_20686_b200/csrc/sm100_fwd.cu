@@ -333,10 +333,10 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK) ||
         !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane(&tB, bias_qk, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
-    // Default: this file's kernel (2 CTAs/SM, 1.95 ms at cfg4).  TRI_FWD_WS=1 selects the warp-specialised two-slot
-    // kernel of sm100_fwd2.cu (2.20 ms at cfg4; kept for A/B and as the base of the next round's pipelining work).
+    // Default: this file's kernel (2 CTAs/SM, 1.82 ms at cfg4).  TRI_FWD_WS=1 selects the warp-specialised kernel of
+    // sm100_fwd3.cu (1 CTA/SM, softmax warpgroups + issuer warps, setmaxnreg; 1.92 ms at cfg4), kept for A/B.
     static const bool ws_kernel = getenv("TRI_FWD_WS") != nullptr;
-    if (ws_kernel) return sm100_fwd2_launch(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
+    if (ws_kernel) return sm100_fwd3_launch(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
     return launch_fwd<4>(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
 }
 
