@@ -250,6 +250,13 @@ def run_ours(args, cfg):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    if not os.path.exists(tri.binding.LIB_PATH):  # fresh checkout: compile the library in-tree first (a build step, not a fallback)
+        from paper_2506_20686_b200 import build as _build
+
+        if rank == 0:
+            _build.build()
+        if world > 1:
+            dist.barrier()
     tri.load()
     peaks = load_peaks()
 
