@@ -234,3 +234,10 @@ def test_alternate_kernels_parity(tri):
     env = dict(os.environ, TRI_FWD_WS="1", TRI_DQ_WS="1")
     r = subprocess.run([sys.executable, "-c", _ALT_SCRIPT], cwd=root, env=env, capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "ALT OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
+def test_n2048_beyond_the_configs_sampled(tri, oracle):
+    """A size above BASELINE.json's largest crop (N=2048, 16 key blocks, ending node, ragged tail mask): sampled rows and
+    dBias lines against the oracle -- exercises long tile loops, the dBias row split and 64-bit indexing."""
+    cfg = tri_inputs.small_config(1, 2048, 1, 32, "bf16", ENDING, 1.5, "tail:37", seed=2048)
+    sampled_compare(oracle, cfg, n_rows=1, n_queries=1)
