@@ -177,8 +177,15 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
                     x[c4 * 4] += mv.x; x[c4 * 4 + 1] += mv.y; x[c4 * 4 + 2] += mv.z; x[c4 * 4 + 3] += mv.w;
                 }
             }
+            {   // four independent max chains (ILP), merged at the end
+                float m4[4] = {x[0], x[1], x[2], x[3]};
 #pragma unroll
-            for (int c = 0; c < BK; ++c) mx = fmaxf(mx, x[c]);
+                for (int c = 4; c < BK; c += 4) {
+                    m4[0] = fmaxf(m4[0], x[c]); m4[1] = fmaxf(m4[1], x[c + 1]);
+                    m4[2] = fmaxf(m4[2], x[c + 2]); m4[3] = fmaxf(m4[3], x[c + 3]);
+                }
+                mx = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
+            }
 
             // ---- online softmax with the -inf guard of reading A6 ---------------------------------
             // The running reference m moves only when this tile's maximum exceeds it by more than kLazy (O and l
@@ -190,7 +197,7 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
             const float alpha = bump ? ex2((m_old - m_safe) * kLog2e) : 1.0f;
             const float mneg = -m_safe * kLog2e;
             const uint64_t l2e2 = pack2(kLog2e, kLog2e), mneg2 = pack2(mneg, mneg);
-            uint64_t lacc = pack2(0.0f, 0.0f);
+            uint64_t lacc4[4] = {pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f)};  // 4 chains (ILP)
 #pragma unroll
             for (int c16 = 0; c16 < BK / 32; ++c16) {  // 32 keys -> 16 packed columns per store
                 uint32_t pk[16];
@@ -199,13 +206,13 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
                     float a0, a1;
                     unpack2(fma2(pack2(x[c16 * 32 + 2 * e], x[c16 * 32 + 2 * e + 1]), l2e2, mneg2), a0, a1);
                     const float p0 = ex2(a0), p1 = ex2(a1);
-                    lacc = add2(lacc, pack2(p0, p1));
+                    lacc4[e & 3] = add2(lacc4[e & 3], pack2(p0, p1));
                     pk[e] = pack_bf16(p0, p1);
                 }
                 tmem_st16(tS + lane_off + c16 * 16, pk);
             }
             float l0, l1;
-            unpack2(lacc, l0, l1);
+            unpack2(add2(add2(lacc4[0], lacc4[1]), add2(lacc4[2], lacc4[3])), l0, l1);
             const float lsum = l0 + l1;
             l_run[r] = l_run[r] * alpha + lsum;
             m_run[r] = m_new;
