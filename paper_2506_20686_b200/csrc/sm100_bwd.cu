@@ -199,15 +199,15 @@ __global__ void __launch_bounds__(256, 2) sm100_dkdv_kernel(const __grid_constan
                 tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
                 uint4 bv[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sB + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
+                for (int j = 0; j < 4; ++j) bv[j] = lds128(sB + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
                 tmem_ld_wait();
                 uint32_t pp[16], ds[16];
                 if (keep[r]) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const uint32_t w[4] = {bv[j].x, bv[j].y, bv[j].z, bv[j].w};
-                        const float4 n0 = *(const float4*)(nlq + c32 * 32 + j * 8), n1 = *(const float4*)(nlq + c32 * 32 + j * 8 + 4);
-                        const float4 d0 = *(const float4*)(ddq + c32 * 32 + j * 8), d1 = *(const float4*)(ddq + c32 * 32 + j * 8 + 4);
+                        const float4 n0 = lds128f(nlq + c32 * 32 + j * 8), n1 = lds128f(nlq + c32 * 32 + j * 8 + 4);
+                        const float4 d0 = lds128f(ddq + c32 * 32 + j * 8), d1 = lds128f(ddq + c32 * 32 + j * 8 + 4);
                         const uint64_t nn[4] = {pack2(n0.x, n0.y), pack2(n0.z, n0.w), pack2(n1.x, n1.y), pack2(n1.z, n1.w)};
                         const uint64_t dn[4] = {pack2(d0.x, d0.y), pack2(d0.z, d0.w), pack2(d1.x, d1.y), pack2(d1.z, d1.w)};
 #pragma unroll
@@ -419,13 +419,13 @@ __global__ void __launch_bounds__(256, 2) sm100_dq_kernel(const __grid_constant_
                 tmem_ld32(tDP + lane_off + c32 * 32, dpraw);
                 uint4 bv[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sBias + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
+                for (int j = 0; j < 4; ++j) bv[j] = lds128(sBias + row * 128 + (((c32 * 4 + j) ^ (row & 7)) << 4));
                 tmem_ld_wait();
                 uint32_t ds[16];
                 if (anymask) {
 #pragma unroll
                     for (int c4 = 0; c4 < 8; ++c4) {
-                        const float4 mv = *(const float4*)(mrow + c32 * 32 + c4 * 4);
+                        const float4 mv = lds128f(mrow + c32 * 32 + c4 * 4);
                         sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);  // -inf survives the scale
                         sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
                         sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);
@@ -646,12 +646,12 @@ __global__ void __launch_bounds__(288, 1) sm100_dbias_kernel(const __grid_consta
                 uint4 bv[4];
 #pragma unroll
                 for (int jj = 0; jj < 4; ++jj)
-                    bv[jj] = *(const uint4*)(sBias + half * 16384 + qrow * 128 + (((c32 * 4 + jj) ^ (qrow & 7)) << 4));
+                    bv[jj] = lds128(sBias + half * 16384 + qrow * 128 + (((c32 * 4 + jj) ^ (qrow & 7)) << 4));
                 tmem_ld_wait();
                 if (anymask) {
 #pragma unroll
                     for (int c4 = 0; c4 < 8; ++c4) {
-                        const float4 mv = *(const float4*)(mrow + c32 * 32 + c4 * 4);
+                        const float4 mv = lds128f(mrow + c32 * 32 + c4 * 4);
                         sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);
                         sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
                         sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);

@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int c = (c32 & 1) * 4 + j;
-                    bv[j] = *(const uint4*)(brow + ((c ^ (tid & 7)) << 4));
+                    bv[j] = lds128(brow + ((c ^ (tid & 7)) << 4));
                 }
                 tmem_ld_wait();
 #pragma unroll
