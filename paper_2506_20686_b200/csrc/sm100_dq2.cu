@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
             const uint8_t* sB = sBias + (kt & 1) * 16384;
             uint4 bv[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) bv[j] = *(const uint4*)(sB + row * 128 + (((chalf * 4 + j) ^ (row & 7)) << 4));
+            for (int j = 0; j < 4; ++j) bv[j] = lds128(sB + row * 128 + (((chalf * 4 + j) ^ (row & 7)) << 4));
             tmem_ld_wait();
             tc_fence_before();
             named_bar_sync(bar_id, 256);  // [A] the whole tile is in registers: S / dP may be overwritten
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
                 const float* mrow = sMask + (t & 1) * 64 + chalf * 32;
 #pragma unroll
                 for (int c4 = 0; c4 < 8; ++c4) {
-                    const float4 mv = *(const float4*)(mrow + c4 * 4);
+                    const float4 mv = lds128f(mrow + c4 * 4);
                     sraw[c4 * 4] = __float_as_uint(__uint_as_float(sraw[c4 * 4]) + mv.x);  // -inf survives the scale
                     sraw[c4 * 4 + 1] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 1]) + mv.y);
                     sraw[c4 * 4 + 2] = __float_as_uint(__uint_as_float(sraw[c4 * 4 + 2]) + mv.z);

@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ 
                 const float4* mrow = (const float4*)(sMask + st * BK);
 #pragma unroll
                 for (int c4 = 0; c4 < BK / 4; ++c4) {
-                    const float4 mv = mrow[c4];
+                    const float4 mv = lds128f(mrow + c4);
                     x[c4 * 4] += mv.x; x[c4 * 4 + 1] += mv.y; x[c4 * 4 + 2] += mv.z; x[c4 * 4 + 3] += mv.w;
                 }
             }

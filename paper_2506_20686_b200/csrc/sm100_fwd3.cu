@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) sm100_fwd3_kernel(const __grid_co
                 const uint8_t* brow = sBias + (kb & 1) * 32768 + row * 128;
 #pragma unroll
                 for (int j = 0; j < 16; ++j) {
-                    const uint4 bv = *(const uint4*)(brow + (j >> 3) * 16384 + (((j & 7) ^ (row & 7)) << 4));
+                    const uint4 bv = lds128(brow + (j >> 3) * 16384 + (((j & 7) ^ (row & 7)) << 4));
                     const uint32_t w[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) sm100_fwd3_kernel(const __grid_co
                     const float4* mrow = (const float4*)(maskS + st * 128);
 #pragma unroll
                     for (int c4 = 0; c4 < BK / 4; ++c4) {
-                        const float4 mv = mrow[c4];
+                        const float4 mv = lds128f(mrow + c4);
                         x[c4 * 4] += mv.x; x[c4 * 4 + 1] += mv.y; x[c4 * 4 + 2] += mv.z; x[c4 * 4 + 3] += mv.w;
                     }
                 }
