@@ -796,13 +796,10 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
               make_tmap_plane(&tBqk, bias_qk, p.B * p.H, p.N, 128) && make_tmap_plane(&tBkq, bias_kq, p.B * p.H, p.N, 128);
     if (!ok) return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
 
-    static bool attr_done = false;
-    if (!attr_done) {
-        if ((s = set_smem(sm100_dkdv_kernel<RKV>, DkdvSmem<RKV>::total)) != TRI_OK) return s;
-        if ((s = set_smem(sm100_dq_kernel<RQ>, DqSmem<RQ>::total)) != TRI_OK) return s;
-        if ((s = set_smem(sm100_dbias_kernel, DbiasSmem::total)) != TRI_OK) return s;
-        attr_done = true;
-    }
+    // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
+    if ((s = set_smem(sm100_dkdv_kernel<RKV>, DkdvSmem<RKV>::total)) != TRI_OK) return s;
+    if ((s = set_smem(sm100_dq_kernel<RQ>, DqSmem<RQ>::total)) != TRI_OK) return s;
+    if ((s = set_smem(sm100_dbias_kernel, DbiasSmem::total)) != TRI_OK) return s;
     {
         ProfScope ps("sm100_dkdv_kernel", st);
         const unsigned grid = (unsigned)((long long)p.B * (p.N / RKV) * p.H * (p.N / 128));

@@ -262,11 +262,8 @@ __global__ void __launch_bounds__(512, 1) sm100_dq2_kernel(const __grid_constant
 tri_status sm100_dq2_launch(const Problem& p, const CUtensorMap& tQ128, const CUtensorMap& tA128, const CUtensorMap& tK64,
                             const CUtensorMap& tV64, const CUtensorMap& tBqk, const unsigned char* mask, const float* LSE,
                             const float* Dws, void* dQ, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
-        TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_dq2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Dq2Smem::total));
-        attr_done = true;
-    }
+    // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
+    TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_dq2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Dq2Smem::total));
     const unsigned grid = (unsigned)((long long)p.B * (p.N / RT) * p.H * (p.N / 128));
     {
         ProfScope ps("sm100_dq2_kernel", st);

@@ -313,11 +313,8 @@ static tri_status launch_fwd(const Problem& p, const CUtensorMap& tQ, const CUte
                              cudaStream_t st) {
     auto kern = sm100_fwd_kernel<R_>;
     const int smem = FwdSmem<R_>::total;
-    static bool attr_done = false;
-    if (!attr_done) {
-        TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_done = true;
-    }
+    // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
+    TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     const unsigned grid = (unsigned)((long long)p.B * (p.N / R_) * p.H * (p.N / BQ));
     {
         ProfScope ps("sm100_fwd_kernel", st);

@@ -315,11 +315,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) sm100_fwd3_kernel(const __grid_co
 tri_status sm100_fwd3_launch(const Problem& p, const CUtensorMap& tQ, const CUtensorMap& tK, const CUtensorMap& tV,
                              const CUtensorMap& tB, const void* G, const unsigned char* mask, void* O, float* LSE,
                              cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
-        TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, F3Smem::total));
-        attr_done = true;
-    }
+    // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
+    TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, F3Smem::total));
     const unsigned grid = (unsigned)((long long)p.B * (p.N / RT) * p.H * (p.N / BQ));
     {
         ProfScope ps("sm100_fwd3_kernel", st);
