@@ -241,3 +241,10 @@ def test_n2048_beyond_the_configs_sampled(tri, oracle):
     dBias lines against the oracle -- exercises long tile loops, the dBias row split and 64-bit indexing."""
     cfg = tri_inputs.small_config(1, 2048, 1, 32, "bf16", ENDING, 1.5, "tail:37", seed=2048)
     sampled_compare(oracle, cfg, n_rows=1, n_queries=1)
+
+
+@pytest.mark.parametrize("variant", [STARTING, ENDING])
+def test_bf16_odd_batch_and_head_counts_full(tri, oracle, variant):
+    """B=3, H=3 (not powers of two) on the tensor-core path, N=128: block-index decoding and per-(b,h) bias planes."""
+    cfg = tri_inputs.small_config(3, 128, 3, 32, "bf16", variant, 1.0, "lengths:100,128,77", seed=333)
+    full_compare(oracle, cfg)
