@@ -8,8 +8,6 @@
 //   dbias    tile-stationary: one CTA owns a 128x128 tile of dBias in registers and streams over ALL broadcast
 //            rows in ascending order (S, dP double-buffered in TMEM) -- deterministic, replaces the paper's
 //            tl.atomic_add; workspace stays O(N^2 H d).
-#include <stdlib.h>
-
 #include "sm100_common.cuh"
 #include "tri_common.cuh"
 
@@ -807,20 +805,13 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
                                                                        (__nv_bfloat16*)dK, (__nv_bfloat16*)dV);
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
-    // Default: sm100_dq_kernel (2 CTAs/SM, 1.96 ms at cfg4).  TRI_DQ_WS=1 selects the two-slot software-pipelined kernel of
-    // sm100_dq2.cu (2.37 ms at cfg4), kept for A/B.
-    static const bool dq_ws = getenv("TRI_DQ_WS") != nullptr;
-    if (!dq_ws) {
-        {
-            ProfScope ps("sm100_dq_kernel", st);
-            const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
-            sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
-                                                                     (__nv_bfloat16*)dQ);
-        }
-        TRI_LAUNCH_CHECK("sm100_dq_kernel");
-    } else {
-        if ((s = sm100_dq2_launch(p, tQ128, tA128, tK64, tV64, tBqk, mask, LSE, Dws, dQ, st)) != TRI_OK) return s;
+    {
+        ProfScope ps("sm100_dq_kernel", st);
+        const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
+        sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
+                                                                 (__nv_bfloat16*)dQ);
     }
+    TRI_LAUNCH_CHECK("sm100_dq_kernel");
     float* planes = (float*)((char*)ws + w.planes_off);
     {
         ProfScope ps("sm100_dbias_kernel", st);

@@ -216,6 +216,20 @@ __device__ __forceinline__ int named_bar_or(int id, int nthreads, int pred) {
     return (int)out;
 }
 
+// ---- register re-allocation between warpgroups (all warps of the warpgroup execute it) -------------------------
+template <int REGS>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS)); }
+template <int REGS>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS)); }
+
+// one arrival per warp: the warp's tcgen05 / shared-memory accesses are ordered before the arrive of lane 0
+__device__ __forceinline__ void warp_arrive(uint64_t* bar) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
+}
+
+__device__ __forceinline__ uint64_t ldg_u64(const unsigned long long* p) { return (uint64_t)__ldg(p); }
+
 // ---- small math helpers ----------------------------------------------------------------------------
 __device__ __forceinline__ float ex2(float x) {
     float y;
@@ -265,11 +279,4 @@ bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d,
 // 3-D map over a [BH, N, N] bf16 plane stack, dims (col, row, bh); box = {64, box_rows, 1}, SWIZZLE_128B.
 bool make_tmap_plane(CUtensorMap* out, const void* base, int BH, int N, int box_rows);
 
-struct Problem;
-tri_status sm100_dq2_launch(const Problem& p, const CUtensorMap& tQ128, const CUtensorMap& tA128, const CUtensorMap& tK64,
-                            const CUtensorMap& tV64, const CUtensorMap& tBqk, const unsigned char* mask, const float* LSE,
-                            const float* Dws, void* dQ, cudaStream_t st);
-tri_status sm100_fwd3_launch(const Problem& p, const CUtensorMap& tQ, const CUtensorMap& tK, const CUtensorMap& tV,
-                             const CUtensorMap& tB, const void* G, const unsigned char* mask, void* O, float* LSE,
-                             cudaStream_t st);
 }  // namespace tri

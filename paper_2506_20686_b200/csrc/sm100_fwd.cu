@@ -1,15 +1,19 @@
 // bf16 forward on tcgen05 / TMEM / TMA (sm_100a): flash-style online softmax, the [B,N,H,N,N] map never leaves
 // the SM (Listing 1, Sec. IV-A; gate, mask and 1/sqrt(d) from the task statement).
 //
-// One CTA (128 threads = 128 query rows, one TMEM lane each) owns a 128-query block of R_ broadcast rows of one
-// (b,h) and walks the key blocks kb = 0..N/128-1 in the OUTER loop and its R_ rows in the INNER loop, so one
-// 128x128 bias tile (TMA, SWIZZLE_128B) serves R_ score tiles ("on-the-fly broadcasting").  Per tile:
-//   S = Q_r K_r^T        tcgen05.mma SS, M=128 N=128 K=2x16, operands TMA-staged (SWIZZLE_64B, K-major)
-//   x = scale*S + bias (+ -inf mask); online max / sum; p = exp2((x - m) log2e)                            P:L166-177
-//   P -> bf16 -> TMEM (aliases S);  O_r += P V_r   tcgen05.mma TS, M=128 N=32 K=8x16, V MN-major
-// Epilogue: O = sigmoid(G) * O_r / l, LSE = m + ln l.
-#include <stdlib.h>
-
+// Persistent, warp-specialised: one CTA per SM, 640 threads =
+//   4 softmax warpgroups ("groups", 128 threads = 128 query rows = 128 TMEM lanes each) -- group g owns broadcast
+//     row 4*rq + g of the current work item (b, h, 128-query block qb, row quad rq) and walks its 64-key tiles;
+//   1 helper warpgroup: warp 16 = TMA producer, warp 17 = tcgen05.mma issuer (one elected lane), warps 18-19 idle.
+// Registers are moved from the helpers to the softmax warpgroups with setmaxnreg.  The four groups of a CTA work on
+// the same (b, h, qb), so one 128x64 bias tile (TMA, SWIZZLE_128B) serves four score tiles ("on-the-fly
+// broadcasting").  Per (group, tile) with TMEM columns [128g, 128g+128) = S 64 | P 32 | O 32:
+//   S = Q_r K_r^T          tcgen05.mma SS, M=128 N=64 K=2x16, operands TMA-staged (SWIZZLE_64B, K-major)
+//   x = scale*S + bias (+ -inf mask); online max / sum; p = exp2((x - m) log2e)                             P:L166-177
+//   P -> bf16 -> TMEM;  O_r += P V_r   tcgen05.mma TS, M=128 N=32 K=4x16, V MN-major
+// S of tile n+1 is issued as soon as the group has S of tile n in registers ("consumed"), so the tensor pipe runs
+// one tile ahead of the softmax and no group waits for an MMA in steady state.
+// Row epilogue: O = sigmoid(G) * O_r / l, LSE = m + ln l.
 #include "sm100_common.cuh"
 #include "tri_common.cuh"
 
@@ -18,268 +22,325 @@ using namespace sm100;
 
 namespace {
 
-constexpr int BQ = 128, BK = 128, DH = 32;
-constexpr int TILE_BYTES = BQ * DH * 2;  // 8 KB: one 128 x 32 bf16 tile
-constexpr float kLazy = 5.0f;            // lazy-rescale threshold on the running max (natural-log units)
+constexpr int NG = 4;                      // softmax groups per CTA
+constexpr int BQ = 128, BK = 64, DH = 32;
+constexpr int KV_ST = 3;                   // K/V ring stages per group
+constexpr int NB = 3;                      // bias ring stages (shared by the groups)
+constexpr int QT_BYTES = BQ * DH * 2;      // 8 KB: 128 x 32 bf16
+constexpr int KT_BYTES = BK * DH * 2;      // 4 KB:  64 x 32 bf16
+constexpr int BIAS_BYTES = BQ * BK * 2;    // 16 KB: [128 q][64 k] bf16, SWIZZLE_128B
+constexpr float kLazy = 5.0f;              // lazy-rescale threshold on the running max (natural-log units)
+constexpr int FWD_THREADS = (NG + 1) * 128;
 
-template <int R_>
 struct FwdSmem {
-    static constexpr int q_off = 0;
-    static constexpr int kv_off = q_off + R_ * TILE_BYTES;       // 2 stages x (K, V)
-    static constexpr int bias_off = kv_off + 4 * TILE_BYTES;     // 2 x 16 KB (key halves), SWIZZLE_128B
-    static constexpr int mask_off = bias_off + 2 * 16384;        // 2 x 128 floats
-    static constexpr int bar_off = mask_off + 2 * BK * 4;        // mbarriers
-    static constexpr int total = bar_off + 64 + 1024;            // + alignment slack
+    static constexpr int q_off = 0;                                    // NG x 2 x Q tile
+    static constexpr int kv_off = q_off + NG * 2 * QT_BYTES;           // NG x KV_ST x (K, V)
+    static constexpr int bias_off = kv_off + NG * KV_ST * 2 * KT_BYTES;
+    static constexpr int bar_off = bias_off + NB * BIAS_BYTES;
+    // mbarriers (8 bytes each)
+    static constexpr int b_kv_full = 0;                                // [NG][KV_ST]
+    static constexpr int b_kv_free = b_kv_full + NG * KV_ST;           // [NG][KV_ST]
+    static constexpr int b_bias_full = b_kv_free + NG * KV_ST;         // [NB]
+    static constexpr int b_bias_free = b_bias_full + NB;               // [NB]
+    static constexpr int b_s_full = b_bias_free + NB;                  // [NG]
+    static constexpr int b_consumed = b_s_full + NG;                   // [NG]
+    static constexpr int b_p_ready = b_consumed + NG;                  // [NG]
+    static constexpr int b_pv_done = b_p_ready + NG;                   // [NG]
+    static constexpr int n_bars = b_pv_done + NG;
+    static constexpr int total = bar_off + n_bars * 8 + 16 + 1024;     // + tmem slot + alignment slack
 };
 
-template <int R_>
-constexpr int tmem_cols() { return (128 + 32 * R_) <= 256 ? 256 : 512; }
+#ifdef TRI_DEBUG_MB
+__device__ unsigned long long g_dbg_mb[1 << 16];
+#endif
+struct Item { int b, h, q0, r4; };
+__device__ __forceinline__ Item decode_item(int item, int N, int H) {
+    const int NRQ = N / NG, NQB = N / BQ;
+    Item it;
+    it.r4 = (item % NRQ) * NG;
+    int t = item / NRQ;
+    it.q0 = (t % NQB) * BQ;
+    const int bh = t / NQB;
+    it.b = bh / H;
+    it.h = bh % H;
+    return it;
+}
 
-template <int R_>
-__global__ void __launch_bounds__(128) sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ,
-                                                        const __grid_constant__ CUtensorMap tmK,
-                                                        const __grid_constant__ CUtensorMap tmV,
-                                                        const __grid_constant__ CUtensorMap tmBias, Problem p,
-                                                        const __nv_bfloat16* __restrict__ G,
-                                                        const unsigned char* __restrict__ mask,
-                                                        __nv_bfloat16* __restrict__ O, float* __restrict__ LSE) {
-    using L = FwdSmem<R_>;
+__global__ void __launch_bounds__(FWD_THREADS, 1)
+sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmBias, Problem p,
+                 const __nv_bfloat16* __restrict__ G, const unsigned long long* __restrict__ maskbits,
+                 __nv_bfloat16* __restrict__ O, float* __restrict__ LSE, int total_items) {
+    using L = FwdSmem;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t* sQ = smem + L::q_off;
     uint8_t* sKV = smem + L::kv_off;
     uint8_t* sBias = smem + L::bias_off;
-    float* sMask = (float*)(smem + L::mask_off);
     uint64_t* bars = (uint64_t*)(smem + L::bar_off);
-    uint64_t* bar_q = bars + 0;
-    uint64_t* bar_kv = bars + 1;  // [2]
-    uint64_t* bar_bias = bars + 3;
-    uint64_t* bar_mma = bars + 4;
-    uint32_t* tmem_slot = (uint32_t*)(bars + 5);
+    uint64_t* kv_full = bars + L::b_kv_full;
+    uint64_t* kv_free = bars + L::b_kv_free;
+    uint64_t* bias_full = bars + L::b_bias_full;
+    uint64_t* bias_free = bars + L::b_bias_free;
+    uint64_t* s_full = bars + L::b_s_full;
+    uint64_t* consumed = bars + L::b_consumed;
+    uint64_t* p_ready = bars + L::b_p_ready;
+    uint64_t* pv_done = bars + L::b_pv_done;
+    uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5;
-    const int NQB = p.N / BQ, NKB = p.N / BK, NG = p.N / R_;
-    int idx = blockIdx.x;
-    const int qb = idx % NQB; idx /= NQB;
-    const int h = idx % p.H; idx /= p.H;
-    const int g = idx % NG;
-    const int b = idx / NG;
-    const int r0 = g * R_, q0 = qb * BQ;
-    const int bh = b * p.H + h;
+    const int N = p.N;
+    const int TPR = N / BK;  // key tiles per row
+    const int n_items = (total_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int NT_all = n_items * TPR;  // tiles per group over the CTA's life
 
     if (tid == 0) {
         prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV); prefetch_tmap(&tmBias);
-        mbar_init(bar_q, 1); mbar_init(bar_kv, 1); mbar_init(bar_kv + 1, 1); mbar_init(bar_bias, 1); mbar_init(bar_mma, 1);
+        for (int i = 0; i < NG * KV_ST; ++i) { mbar_init(kv_full + i, 1); mbar_init(kv_free + i, 1); }
+        for (int i = 0; i < NB; ++i) { mbar_init(bias_full + i, 1); mbar_init(bias_free + i, NG * 4); }
+        for (int i = 0; i < NG; ++i) {
+            mbar_init(s_full + i, 1); mbar_init(consumed + i, 4); mbar_init(p_ready + i, 4); mbar_init(pv_done + i, 1);
+        }
         fence_barrier_init();
     }
-    if (warp == 0) tmem_alloc<tmem_cols<R_>()>(tmem_slot);
+    if (warp == 0) tmem_alloc<512>(tmem_slot);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t tS = tmem;                                  // S: columns [0,128); P (bf16 pairs): [0,64)
-    const uint32_t lane_off = (uint32_t)(warp * 32) << 16;      // this warp's TMEM lane quarter
-    const int T = NKB * R_;
 
-    auto load_kv = [&](int t) {
-        const int kb = t / R_, r = t % R_, st = t & 1;
-        mbar_expect_tx(bar_kv + st, 2 * TILE_BYTES);
-        tma_load_5d(sKV + st * 2 * TILE_BYTES, &tmK, bar_kv + st, 0, kb * BK, r0 + r, h, b);
-        tma_load_5d(sKV + st * 2 * TILE_BYTES + TILE_BYTES, &tmV, bar_kv + st, 0, kb * BK, r0 + r, h, b);
-    };
-    auto load_bias = [&](int kb) {
-        mbar_expect_tx(bar_bias, 2 * 16384);
-        tma_load_3d(sBias, &tmBias, bar_bias, kb * BK, q0, bh);
-        tma_load_3d(sBias + 16384, &tmBias, bar_bias, kb * BK + 64, q0, bh);
-    };
-    if (tid == 0) {
-        mbar_expect_tx(bar_q, R_ * TILE_BYTES);
-        for (int r = 0; r < R_; ++r) tma_load_5d(sQ + r * TILE_BYTES, &tmQ, bar_q, 0, q0, r0 + r, h, b);
-        load_kv(0);
-        load_bias(0);
-    }
-    // mask for tile t: keep flag of key (kb*128 + tid) in row r0 + r
-    auto mask_val = [&](int t) -> float {
-        const int kb = t / R_, r = t % R_;
-        const unsigned char mk = mask[(long long)b * p.N * p.N + (long long)(r0 + r) * p.mR + (long long)(kb * BK + tid) * p.mK];
-        return mk ? 0.0f : -INFINITY;
-    };
-    int anymask = 0;
-    if (mask) {
-        const float mv = mask_val(0);
-        sMask[tid] = mv;
-        anymask = __syncthreads_or(mv != 0.0f);
-    }
-
-    constexpr uint32_t idescS = make_idesc(128, 128, false, false);
-    constexpr uint32_t idescO = make_idesc(128, DH, false, true);
-    const float scale = rsqrtf((float)DH);
-    const uint64_t scale2 = pack2(scale, scale);
-    float m_run[R_], l_run[R_];
-#pragma unroll
-    for (int r = 0; r < R_; ++r) { m_run[r] = -INFINITY; l_run[r] = 0.0f; }
-
-    for (int kb = 0; kb < NKB; ++kb) {
-#pragma unroll
-        for (int r = 0; r < R_; ++r) {
-            const int t = kb * R_ + r, st = t & 1;
-            if (warp == 0) {  // warp-uniform so the descriptors stay in uniform registers; one elected lane issues
-                if (t == 0) mbar_wait(bar_q, 0);
-                mbar_wait(bar_kv + st, (t >> 1) & 1);
-                tc_fence_after();
-                const uint64_t dq = make_desc_sw64(smem_u32(sQ + r * TILE_BYTES));
-                const uint64_t dk = make_desc_sw64(smem_u32(sKV + st * 2 * TILE_BYTES));
-                if (elect_one()) {
-                    mma_ss(tS, dq, dk, idescS, 0);
-                    mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-                    mma_commit(bar_mma);
+    if (warp >= NG * 4) {
+        // =============================== helper warpgroup ===============================
+#ifndef TRI_NO_SETMAXNREG
+        setmaxnreg_dec<40>();
+#endif
+        if (warp == NG * 4) {
+            // ---- TMA producer: bias tile of (item, kt) once, then (Q at kt = 0,) K, V of every group ----
+            int kst = 0, kph = 0, bst = 0, bph = 0;
+            for (int il = 0; il < n_items; ++il) {
+                const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H);
+                const int bh = it.b * p.H + it.h;
+                for (int kt = 0; kt < TPR; ++kt) {
+                    mbar_wait(bias_free + bst, bph ^ 1);
+                    if (elect_one()) {
+                        mbar_expect_tx(bias_full + bst, BIAS_BYTES);
+                        tma_load_3d(sBias + bst * BIAS_BYTES, &tmBias, bias_full + bst, kt * BK, it.q0, bh);
+                    }
+                    __syncwarp();
+#pragma unroll 1
+                    for (int g = 0; g < NG; ++g) {
+                        uint64_t* full = kv_full + g * KV_ST + kst;
+                        mbar_wait(kv_free + g * KV_ST + kst, kph ^ 1);
+                        if (elect_one()) {
+                            uint8_t* kv = sKV + (g * KV_ST + kst) * 2 * KT_BYTES;
+                            mbar_expect_tx(full, 2 * KT_BYTES + (kt == 0 ? QT_BYTES : 0));
+                            if (kt == 0) tma_load_5d(sQ + (g * 2 + (il & 1)) * QT_BYTES, &tmQ, full, 0, it.q0, it.r4 + g, it.h, it.b);
+                            tma_load_5d(kv, &tmK, full, 0, kt * BK, it.r4 + g, it.h, it.b);
+                            tma_load_5d(kv + KT_BYTES, &tmV, full, 0, kt * BK, it.r4 + g, it.h, it.b);
+                        }
+                        __syncwarp();
+                    }
+                    if (++kst == KV_ST) { kst = 0; kph ^= 1; }
+                    if (++bst == NB) { bst = 0; bph ^= 1; }
                 }
-                __syncwarp();
             }
-            float mnext = 0.0f;
-            if (mask && t + 1 < T) mnext = mask_val(t + 1);
-            mbar_wait(bar_mma, t & 1);
-            tc_fence_after();
-            if (tid == 32 && t + 1 < T) load_kv(t + 1);  // (warp 1: warp 0 carries the MMA issue) stage (t+1)&1 was last read by tile t-1
-            if (r == 0) mbar_wait(bar_bias, kb & 1);
-
-            // ---- scores of my query row: x = scale*S + bias (+ mask) ---------------------------------------
-            float x[BK];
-            float mx = -INFINITY;
+        } else if (warp == NG * 4 + 1) {
+            // ---- MMA issuer (warp-uniform control flow; one elected lane issues and commits) ----
+            // Polls the groups: a group whose P(n) is ready gets O += P V; a group that has read S(n+1) out of
+            // TMEM gets S(n+2).  No group ever waits for another group's epilogue.
+            constexpr uint32_t idescS = make_idesc(128, BK, false, false);
+            constexpr uint32_t idescO = make_idesc(128, DH, false, true);
+            int s_n[NG], s_st[NG], s_kt[NG], s_il[NG];  // next S tile of group g: index, ring stage, key tile, item parity
+            int p_n[NG], p_st[NG], p_kt[NG];            // next P V tile of group g
 #pragma unroll
-            for (int c32 = 0; c32 < 4; ++c32) {
-                uint32_t raw[32];
-                tmem_ld32(tS + lane_off + c32 * 32, raw);
-                const uint8_t* brow = sBias + (c32 >> 1) * 16384 + tid * 128;
-                uint4 bv[4];
+            for (int g = 0; g < NG; ++g) { s_n[g] = s_st[g] = s_kt[g] = s_il[g] = 0; p_n[g] = p_st[g] = p_kt[g] = 0; }
+            int remaining = NG * NT_all;
+            while (remaining > 0) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int c = (c32 & 1) * 4 + j;
-                    bv[j] = lds128(brow + ((c ^ (tid & 7)) << 4));
-                }
-                tmem_ld_wait();
+                for (int g = 0; g < NG; ++g) {
+                    // S(g, m): needs the S columns free (tile m-1 read out) and K (and Q) of tile m in shared memory
+                    if (s_n[g] < NT_all && (s_n[g] == 0 || mbar_test_wait(consumed + g, (s_n[g] - 1) & 1)) &&
+                        mbar_test_wait(kv_full + g * KV_ST + s_st[g], (s_n[g] / KV_ST) & 1)) {
+                        tc_fence_after();
+                        const uint64_t dq = make_desc_sw64(smem_u32(sQ + (g * 2 + (s_il[g] & 1)) * QT_BYTES));
+                        const uint64_t dk = make_desc_sw64(smem_u32(sKV + (g * KV_ST + s_st[g]) * 2 * KT_BYTES));
+                        const uint32_t tS = tmem + g * 128;
+                        if (elect_one()) {
+                            mma_ss(tS, dq, dk, idescS, 0);
+                            mma_ss(tS, dq + 2, dk + 2, idescS, 1);
+                            mma_commit(s_full + g);
+                        }
+                        __syncwarp();
+                        ++s_n[g];
+                        if (++s_st[g] == KV_ST) s_st[g] = 0;
+                        if (++s_kt[g] == TPR) { s_kt[g] = 0; ++s_il[g]; }
+                    }
+                    // O(g) += P(g, m) V(g, m)
+                    if (p_n[g] < NT_all && mbar_test_wait(p_ready + g, p_n[g] & 1)) {
+                        tc_fence_after();
+                        const uint64_t dv = make_desc_sw64(smem_u32(sKV + (g * KV_ST + p_st[g]) * 2 * KT_BYTES + KT_BYTES));
+                        const uint32_t tP = tmem + g * 128 + 64, tO = tmem + g * 128 + 96;
+                        if (elect_one()) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const uint32_t w[4] = {bv[j].x, bv[j].y, bv[j].z, bv[j].w};
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int col = c32 * 32 + j * 8 + e * 2;
-                        unpack2(fma2(pack2(__uint_as_float(raw[j * 8 + e * 2]), __uint_as_float(raw[j * 8 + e * 2 + 1])), scale2,
-                                     pack2(bf16_lo(w[e]), bf16_hi(w[e]))), x[col], x[col + 1]);
+                            for (int ks = 0; ks < BK / 16; ++ks)
+                                mma_ts(tO, tP + ks * 8, dv + (uint64_t)ks * 64, idescO, (p_kt[g] > 0 || ks > 0) ? 1u : 0u);
+                            mma_commit(kv_free + g * KV_ST + p_st[g]);
+                            mma_commit(pv_done + g);
+                        }
+                        __syncwarp();
+                        ++p_n[g];
+                        --remaining;
+                        if (++p_st[g] == KV_ST) p_st[g] = 0;
+                        if (++p_kt[g] == TPR) p_kt[g] = 0;
                     }
                 }
             }
-            if (anymask) {
-                const float4* mrow = (const float4*)(sMask + st * BK);
-#pragma unroll
-                for (int c4 = 0; c4 < BK / 4; ++c4) {
-                    const float4 mv = lds128f(mrow + c4);
-                    x[c4 * 4] += mv.x; x[c4 * 4 + 1] += mv.y; x[c4 * 4 + 2] += mv.z; x[c4 * 4 + 3] += mv.w;
-                }
-            }
-            {   // four independent max chains (ILP), merged at the end
-                float m4[4] = {x[0], x[1], x[2], x[3]};
-#pragma unroll
-                for (int c = 4; c < BK; c += 4) {
-                    m4[0] = fmaxf(m4[0], x[c]); m4[1] = fmaxf(m4[1], x[c + 1]);
-                    m4[2] = fmaxf(m4[2], x[c + 2]); m4[3] = fmaxf(m4[3], x[c + 3]);
-                }
-                mx = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
-            }
+        }
+    } else {
+        // =============================== softmax groups ===============================
+#ifndef TRI_NO_SETMAXNREG
+        setmaxnreg_inc<104>();  // 512 x 104 + 128 x 40 <= 640 x 96 (the launch allocation)
+#endif
+        const int g = warp >> 2;
+        const int row = tid & 127;                                  // query row inside the block = TMEM lane
+        const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
+        const uint32_t tS = tmem + g * 128 + lane_off, tP = tS + 64, tO = tS + 96;
+        const float scale = rsqrtf((float)DH);
+        const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
+        const int NW = N / 64;  // mask words per row
+        int bst = 0, bph = 0;
+        int n = 0;
+        for (int il = 0; il < n_items; ++il) {
+            const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H);
+            const int r = it.r4 + g;
+            const unsigned long long* mrow = maskbits ? maskbits + ((long long)it.b * N + r) * NW : nullptr;
+            uint64_t mb_next = mrow ? ldg_u64(mrow) : ~0ull;
+            float m_run = -INFINITY, l_run = 0.0f;
+            const long long off = (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)r * p.sSlice + (long long)(it.q0 + row) * p.sPos;
+            for (int kt = 0; kt < TPR; ++kt, ++n) {
+                const uint64_t mb = mb_next;
+                if (mrow && kt + 1 < TPR) mb_next = ldg_u64(mrow + kt + 1);
+#ifdef TRI_DEBUG_MB
+                if ((tid & 31) == 0)
+                    g_dbg_mb[(((((it.b * p.H + it.h) * (N / BQ) + it.q0 / BQ) * N + r) * NW + kt) * 4 + (warp & 3)) & 0xffff] = mb;
+#endif
+                mbar_wait(s_full + g, n & 1);
+                tc_fence_after();
+                uint32_t raw[BK];
+                tmem_ld32(tS, *(uint32_t(*)[32])&raw[0]);
+                tmem_ld32(tS + 32, *(uint32_t(*)[32])&raw[32]);
+                mbar_wait(bias_full + bst, bph);
+                const uint8_t* brow = sBias + bst * BIAS_BYTES + row * 128;
+                tmem_ld_wait();
+                tc_fence_before();
+                warp_arrive(consumed + g);  // S(n) is in registers: the issuer may overwrite the S columns
 
-            // ---- online softmax with the -inf guard of reading A6 ---------------------------------
-            // The running reference m moves only when this tile's maximum exceeds it by more than kLazy (O and l
-            // share the reference, so the result is exact either way): keeps the O rescale out of almost every tile.
-            const float m_old = m_run[r];
-            const bool bump = mx > m_old + kLazy;
-            const float m_new = bump ? mx : m_old;
-            const float m_safe = (m_new == -INFINITY) ? 0.0f : m_new;
-            const float alpha = bump ? ex2((m_old - m_safe) * kLog2e) : 1.0f;
-            const float mneg = -m_safe * kLog2e;
-            const uint64_t l2e2 = pack2(kLog2e, kLog2e), mneg2 = pack2(mneg, mneg);
-            uint64_t lacc4[4] = {pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f)};  // 4 chains (ILP)
+                // ---- scores of my query row: x = scale*S + bias (+ mask) ---------------------------------------
+                float x[BK];
 #pragma unroll
-            for (int c16 = 0; c16 < BK / 32; ++c16) {  // 32 keys -> 16 packed columns per store
-                uint32_t pk[16];
+                for (int c8 = 0; c8 < BK / 8; ++c8) {
+                    const uint4 bv = lds128(brow + ((c8 ^ (row & 7)) << 4));
+                    const uint32_t w[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
-                for (int e = 0; e < 16; ++e) {
+                    for (int e = 0; e < 4; ++e) {
+                        const int c = c8 * 8 + e * 2;
+                        unpack2(fma2(pack2(__uint_as_float(raw[c]), __uint_as_float(raw[c + 1])), scale2,
+                                     pack2(bf16_lo(w[e]), bf16_hi(w[e]))), x[c], x[c + 1]);
+                    }
+                }
+                // my generic-proxy reads of the bias tile must be complete before the producer's TMA (async proxy) may
+                // overwrite it: without the proxy fence the arrive can overtake the ld.shared of a busy warp
+                fence_proxy_async();
+                warp_arrive(bias_free + bst);
+                if (++bst == NB) { bst = 0; bph ^= 1; }
+                if (mb != ~0ull) {
+#pragma unroll
+                    for (int c = 0; c < BK; ++c)
+                        if (!((mb >> c) & 1ull)) x[c] = -INFINITY;
+                }
+                float mx;
+                {   // four independent max chains (ILP), merged at the end
+                    float m4[4] = {x[0], x[1], x[2], x[3]};
+#pragma unroll
+                    for (int c = 4; c < BK; c += 4) {
+                        m4[0] = fmaxf(m4[0], x[c]); m4[1] = fmaxf(m4[1], x[c + 1]);
+                        m4[2] = fmaxf(m4[2], x[c + 2]); m4[3] = fmaxf(m4[3], x[c + 3]);
+                    }
+                    mx = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
+                }
+                // ---- online softmax with the -inf guard of reading A6 ---------------------------------
+                // The running reference m moves only when this tile's maximum exceeds it by more than kLazy (O and l
+                // share the reference, so the result is exact either way): keeps the O rescale out of almost every tile.
+                const float m_old = m_run;
+                const bool bump = mx > m_old + kLazy;
+                const float m_new = bump ? mx : m_old;
+                const float m_safe = (m_new == -INFINITY) ? 0.0f : m_new;
+                const float alpha = bump ? ex2((m_old - m_safe) * kLog2e) : 1.0f;
+                const float mneg = -m_safe * kLog2e;
+                const uint64_t mneg2 = pack2(mneg, mneg);
+                uint64_t lacc4[4] = {pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f)};
+                uint32_t pk[BK / 2];
+#pragma unroll
+                for (int e = 0; e < BK / 2; ++e) {
                     float a0, a1;
-                    unpack2(fma2(pack2(x[c16 * 32 + 2 * e], x[c16 * 32 + 2 * e + 1]), l2e2, mneg2), a0, a1);
+                    unpack2(fma2(pack2(x[2 * e], x[2 * e + 1]), l2e2, mneg2), a0, a1);
                     const float p0 = ex2(a0), p1 = ex2(a1);
                     lacc4[e & 3] = add2(lacc4[e & 3], pack2(p0, p1));
                     pk[e] = pack_bf16(p0, p1);
                 }
-                tmem_st16(tS + lane_off + c16 * 16, pk);
-            }
-            float l0, l1;
-            unpack2(add2(add2(lacc4[0], lacc4[1]), add2(lacc4[2], lacc4[3])), l0, l1);
-            const float lsum = l0 + l1;
-            l_run[r] = l_run[r] * alpha + lsum;
-            m_run[r] = m_new;
-            if (kb > 0 && __any_sync(0xffffffffu, bump)) {  // rescale the accumulator O_r
-                uint32_t o[32];
-                tmem_ld32(tmem + lane_off + 128 + r * 32, o);
-                tmem_ld_wait();
-#pragma unroll
-                for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
-                tmem_st32(tmem + lane_off + 128 + r * 32, o);
-            }
-            if (mask && t + 1 < T) sMask[((t + 1) & 1) * BK + tid] = mnext;
-            tmem_st_wait();
-            tc_fence_before();
-            if (mask) anymask = __syncthreads_or(mnext != 0.0f); else __syncthreads();
-            if (warp == 0) {
-                tc_fence_after();
-                const uint64_t dv = make_desc_sw64(smem_u32(sKV + st * 2 * TILE_BYTES + TILE_BYTES));
-                if (elect_one()) {
-#pragma unroll
-                    for (int ks = 0; ks < BK / 16; ++ks)
-                        mma_ts(tmem + 128 + r * 32, tS + ks * 8, dv + (uint64_t)ks * 64, idescO, (kb > 0 || ks > 0) ? 1u : 0u);
-                    if (r == R_ - 1 && kb + 1 < NKB) load_bias(kb + 1);  // every thread is past its bias reads
+                float l0, l1;
+                unpack2(add2(add2(lacc4[0], lacc4[1]), add2(lacc4[2], lacc4[3])), l0, l1);
+                l_run = l_run * alpha + (l0 + l1);
+                m_run = m_new;
+                // P(n-1) has been read and O(n-1) accumulated before P / O are touched again
+                if (n > 0) {
+                    mbar_wait(pv_done + g, (n - 1) & 1);
+                    tc_fence_after();
                 }
-                __syncwarp();
+                if (kt > 0 && __any_sync(0xffffffffu, bump)) {  // rescale the accumulator O_r
+                    uint32_t o[32];
+                    tmem_ld32(tO, o);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                    tmem_st32(tO, o);
+                }
+                tmem_st32(tP, pk);
+                tmem_st_wait();
+                tc_fence_before();
+                warp_arrive(p_ready + g);
             }
-        }
-    }
-    if (tid == 0) mma_commit(bar_mma);
-    mbar_wait(bar_mma, T & 1);
-    tc_fence_after();
-
-    // ---- epilogue: O = sigmoid(G) * O_r / l ; LSE = m + ln l -------------------------------------------
+            // ---- row epilogue: O = sigmoid(G) * O_r / l ; LSE = m + ln l -------------------------------
+            uint4 gv[4];
+            const uint4* gp = (const uint4*)(G + off);
 #pragma unroll
-    for (int r = 0; r < R_; ++r) {
-        uint32_t o[32];
-        tmem_ld32(tmem + lane_off + 128 + r * 32, o);
-        const long long off = (long long)b * p.sB + (long long)h * p.sH + (long long)(r0 + r) * p.sSlice + (long long)(q0 + tid) * p.sPos;
-        const uint4* gp = (const uint4*)(G + off);
-        uint4 gv[4];
+            for (int j = 0; j < 4; ++j) gv[j] = __ldg(gp + j);
+            mbar_wait(pv_done + g, (n - 1) & 1);
+            tc_fence_after();
+            uint32_t o[32];
+            tmem_ld32(tO, o);
+            tmem_ld_wait();
+            const float inv = l_run > 0.0f ? 1.0f / l_run : 0.0f;
+            uint4* op = (uint4*)(O + off);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) gv[j] = __ldg(gp + j);
-        tmem_ld_wait();
-        const float l = l_run[r];
-        const float inv = l > 0.0f ? 1.0f / l : 0.0f;
-        uint4 ov[4];
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t gw[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
+                uint32_t ow[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t gw[4] = {gv[j].x, gv[j].y, gv[j].z, gv[j].w};
-            uint32_t ow[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const float g0 = bf16_lo(gw[e]), g1 = bf16_hi(gw[e]);
-                const float s0 = __fdividef(1.0f, 1.0f + ex2(-g0 * kLog2e)), s1 = __fdividef(1.0f, 1.0f + ex2(-g1 * kLog2e));
-                ow[e] = pack_bf16(__uint_as_float(o[j * 8 + 2 * e]) * inv * s0, __uint_as_float(o[j * 8 + 2 * e + 1]) * inv * s1);
+                for (int e = 0; e < 4; ++e) {
+                    const float g0 = bf16_lo(gw[e]), g1 = bf16_hi(gw[e]);
+                    const float s0 = __fdividef(1.0f, 1.0f + ex2(-g0 * kLog2e)), s1 = __fdividef(1.0f, 1.0f + ex2(-g1 * kLog2e));
+                    ow[e] = pack_bf16(__uint_as_float(o[j * 8 + 2 * e]) * inv * s0, __uint_as_float(o[j * 8 + 2 * e + 1]) * inv * s1);
+                }
+                op[j] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
-            ov[j] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+            const long long loff = (long long)it.b * N * p.H * N + (long long)it.h * N + (long long)r * p.lR + (long long)(it.q0 + row) * p.lQ;
+            LSE[loff] = l_run > 0.0f ? m_run + __logf(l_run) : -INFINITY;
         }
-        uint4* op = (uint4*)(O + off);
-#pragma unroll
-        for (int j = 0; j < 4; ++j) op[j] = ov[j];
-        const long long loff = (long long)b * p.N * p.H * p.N + (long long)h * p.N + (long long)(r0 + r) * p.lR + (long long)(q0 + tid) * p.lQ;
-        LSE[loff] = l > 0.0f ? m_run[r] + __logf(l) : -INFINITY;
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc<tmem_cols<R_>()>(tmem);
+    if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
 // bf16 plane transpose out[bh][j][i] = in[bh][i][j]  (bias for the ending-node variant: bias[b,h,k,i] -> [q=i][k])
@@ -293,6 +354,29 @@ __global__ void transpose_bf16_kernel(const __nv_bfloat16* __restrict__ in, __nv
     for (int j = threadIdx.y; j < 32; j += 8) out[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
 }
 
+// keep flags [B,N,N] (u8) -> one 64-bit word per (b, row r, 64-key tile): bit k = key 64*w + k of row r is visible.
+// Rows / keys follow the variant (mask element (r,k) at r*mR + k*mK), so the kernels read one word per tile.
+__global__ void __launch_bounds__(128) pack_mask_kernel(const unsigned char* __restrict__ mask,
+                                                        unsigned long long* __restrict__ bits, Problem p) {
+    const int lane = threadIdx.x & 31, w = blockIdx.x * 4 + (threadIdx.x >> 5);
+    const int r = blockIdx.y, b = blockIdx.z, NW = p.N / 64;
+    if (w >= NW) return;
+    const unsigned char* base = mask + (long long)b * p.N * p.N + (long long)r * p.mR;
+    const unsigned lo = __ballot_sync(0xffffffffu, base[(long long)(w * 64 + lane) * p.mK] != 0);
+    const unsigned hi = __ballot_sync(0xffffffffu, base[(long long)(w * 64 + 32 + lane) * p.mK] != 0);
+    if (lane == 0) bits[((long long)b * p.N + r) * NW + w] = (unsigned long long)lo | ((unsigned long long)hi << 32);
+}
+
+int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+            n = 148;
+    }
+    return n;
+}
+
 }  // namespace
 
 tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cudaStream_t st) {
@@ -301,47 +385,60 @@ tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cuda
     return TRI_OK;
 }
 
-bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0; }
-
-size_t sm100_fwd_workspace(const Problem& p) {
-    return p.variant == TRI_ENDING ? align_up((size_t)p.B * p.H * p.N * p.N * 2, 256) : 0;
+tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st) {
+    ProfScope ps("pack_mask_kernel", st);
+    pack_mask_kernel<<<dim3((p.N / 64 + 3) / 4, p.N, p.B), 128, 0, st>>>(mask, (unsigned long long*)bits, p);
+    return TRI_OK;
 }
 
-template <int R_>
-static tri_status launch_fwd(const Problem& p, const CUtensorMap& tQ, const CUtensorMap& tK, const CUtensorMap& tV,
-                             const CUtensorMap& tB, const void* G, const unsigned char* mask, void* O, float* LSE,
-                             cudaStream_t st) {
-    auto kern = sm100_fwd_kernel<R_>;
-    const int smem = FwdSmem<R_>::total;
-    // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
-    TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    const unsigned grid = (unsigned)((long long)p.B * (p.N / R_) * p.H * (p.N / BQ));
-    {
-        ProfScope ps("sm100_fwd_kernel", st);
-        kern<<<grid, 128, smem, st>>>(tQ, tK, tV, tB, p, (const __nv_bfloat16*)G, mask, (__nv_bfloat16*)O, LSE);
-    }
-    TRI_LAUNCH_CHECK("sm100_fwd_kernel");
-    return TRI_OK;
+int sm100_sm_count() { return sm_count(); }
+#ifdef TRI_DEBUG_MB
+extern "C" __attribute__((visibility("default"))) int tri_debug_mb(unsigned long long* host, int n) {
+    return (int)cudaMemcpyFromSymbol(host, g_dbg_mb, (size_t)n * 8);
+}
+#endif
+
+bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0; }
+
+size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.N * (p.N / 64) * 8, 256); }
+
+size_t sm100_fwd_workspace(const Problem& p) {
+    return sm100_maskbits_bytes(p) + (p.variant == TRI_ENDING ? align_up((size_t)p.B * p.H * p.N * p.N * 2, 256) : 0);
 }
 
 tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void* V, const void* G, const void* bias,
                      const unsigned char* mask, void* O, float* LSE, void* ws, cudaStream_t st) {
+    void* maskbits = nullptr;
+    if (mask) {
+        maskbits = ws;
+        tri_status s = sm100_pack_mask(p, mask, maskbits, st);
+        if (s != TRI_OK) return s;
+        TRI_LAUNCH_CHECK("pack_mask_kernel");
+    }
     const void* bias_qk = bias;
     if (p.variant == TRI_ENDING) {
-        tri_status s = sm100_transpose_planes(bias, ws, p.B * p.H, p.N, st);
+        void* biasT = (char*)ws + sm100_maskbits_bytes(p);
+        tri_status s = sm100_transpose_planes(bias, biasT, p.B * p.H, p.N, st);
         if (s != TRI_OK) return s;
         TRI_LAUNCH_CHECK("sm100_transpose_bf16");
-        bias_qk = ws;
+        bias_qk = biasT;
     }
     CUtensorMap tQ, tK, tV, tB;
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK) ||
         !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane(&tB, bias_qk, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
-    // Default: this file's kernel (2 CTAs/SM, 1.82 ms at cfg4).  TRI_FWD_WS=1 selects the warp-specialised kernel of
-    // sm100_fwd3.cu (1 CTA/SM, softmax warpgroups + issuer warps, setmaxnreg; 1.92 ms at cfg4), kept for A/B.
-    static const bool ws_kernel = getenv("TRI_FWD_WS") != nullptr;
-    if (ws_kernel) return sm100_fwd3_launch(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
-    return launch_fwd<4>(p, tQ, tK, tV, tB, G, mask, O, LSE, st);
+    // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
+    TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));
+    const long long items = (long long)p.B * p.H * (p.N / BQ) * (p.N / NG);
+    const int grid = (int)(items < sm_count() ? items : sm_count());
+    {
+        ProfScope ps("sm100_fwd_kernel", st);
+        sm100_fwd_kernel<<<grid, FWD_THREADS, FwdSmem::total, st>>>(tQ, tK, tV, tB, p, (const __nv_bfloat16*)G,
+                                                                    (const unsigned long long*)maskbits,
+                                                                    (__nv_bfloat16*)O, LSE, (int)items);
+    }
+    TRI_LAUNCH_CHECK("sm100_fwd_kernel");
+    return TRI_OK;
 }
 
 }  // namespace tri

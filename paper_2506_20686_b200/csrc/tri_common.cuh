@@ -86,6 +86,10 @@ tri_status simt_bwd(const Problem& p, tri_dtype dt, const void* dO, const void* 
 // ---- bf16 tcgen05 / TMA path (sm100_fwd.cu, sm100_bwd.cu) ------------------------------------
 bool sm100_supported(const Problem& p, tri_dtype dt);
 tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cudaStream_t st);  // bf16 [BH,N,N]
+// keep flags -> one 64-bit word per (b, row, 64-key tile), rows / keys in the variant's sense
+tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st);
+size_t sm100_maskbits_bytes(const Problem& p);
+int sm100_sm_count();
 size_t sm100_fwd_workspace(const Problem& p);
 size_t sm100_bwd_workspace(const Problem& p);
 tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void* V, const void* G,
