@@ -4,7 +4,8 @@
 // Persistent, warp-specialised: one CTA per SM, 640 threads =
 //   4 softmax warpgroups ("groups", 128 threads = 128 query rows = 128 TMEM lanes each) -- group g owns broadcast
 //     row 4*rq + g of the current work item (b, h, 128-query block qb, row quad rq) and walks its 64-key tiles;
-//   1 helper warpgroup: warp 16 = TMA producer, warp 17 = tcgen05.mma issuer (one elected lane), warps 18-19 idle.
+//   1 helper warpgroup: warp 16 = TMA producer, warps 17-18 = tcgen05.mma issuers (two groups each, one elected
+//     lane), warp 19 idle.
 // Registers are moved from the helpers to the softmax warpgroups with setmaxnreg.  The four groups of a CTA work on
 // the same (b, h, qb), so one 128x64 bias tile (TMA, SWIZZLE_128B) serves four score tiles ("on-the-fly
 // broadcasting").  Per (group, tile) with TMEM columns [128g, 128g+128) = S 64 | P 32 | O 32:
@@ -144,26 +145,55 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                     if (++bst == NB) { bst = 0; bph ^= 1; }
                 }
             }
-        } else if (warp == NG * 4 + 1) {
-            // ---- MMA issuer (warp-uniform control flow; one elected lane issues and commits) ----
-            // Polls the groups: a group whose P(n) is ready gets O += P V; a group that has read S(n+1) out of
-            // TMEM gets S(n+2).  No group ever waits for another group's epilogue.
+        } else if (warp == NG * 4 + 1 || warp == NG * 4 + 2) {
+            // ---- MMA issuers (warp-uniform control flow; one elected lane issues and commits) ----
+            // Warp 17 serves groups 0-1, warp 18 groups 2-3.  Each polls its groups: a group whose P(n) is ready gets
+            // O += P V; a group that has read S(n+1) out of TMEM gets S(n+2).  No group waits for another's epilogue.
+            constexpr int NGI = NG / 2;
+            const int g0 = (warp - (NG * 4 + 1)) * NGI;
             constexpr uint32_t idescS = make_idesc(128, BK, false, false);
             constexpr uint32_t idescO = make_idesc(128, DH, false, true);
-            int s_n[NG], s_st[NG], s_kt[NG], s_il[NG];  // next S tile of group g: index, ring stage, key tile, item parity
-            int p_n[NG], p_st[NG], p_kt[NG];            // next P V tile of group g
+            int s_n[NGI], s_st[NGI], s_kt[NGI], s_par[NGI];  // next S tile: index, ring stage, key tile, Q buffer
+            int p_n[NGI], p_st[NGI], p_kt[NGI];              // next P V tile
 #pragma unroll
-            for (int g = 0; g < NG; ++g) { s_n[g] = s_st[g] = s_kt[g] = s_il[g] = 0; p_n[g] = p_st[g] = p_kt[g] = 0; }
-            int remaining = NG * NT_all;
+            for (int j = 0; j < NGI; ++j) { s_n[j] = s_st[j] = s_kt[j] = s_par[j] = 0; p_n[j] = p_st[j] = p_kt[j] = 0; }
+            const uint32_t qbase = smem_u32(sQ), kvbase = smem_u32(sKV);
+            int remaining = NGI * NT_all;
             while (remaining > 0) {
+                // probe every barrier first (the probes are independent and overlap), then act
+                bool okS[NGI], okP[NGI];
 #pragma unroll
-                for (int g = 0; g < NG; ++g) {
-                    // S(g, m): needs the S columns free (tile m-1 read out) and K (and Q) of tile m in shared memory
-                    if (s_n[g] < NT_all && (s_n[g] == 0 || mbar_test_wait(consumed + g, (s_n[g] - 1) & 1)) &&
-                        mbar_test_wait(kv_full + g * KV_ST + s_st[g], (s_n[g] / KV_ST) & 1)) {
+                for (int j = 0; j < NGI; ++j) {
+                    const int g = g0 + j;
+                    const bool c = s_n[j] == 0 || mbar_test_wait(consumed + g, (s_n[j] - 1) & 1);
+                    const bool k = mbar_test_wait(kv_full + g * KV_ST + s_st[j], (s_n[j] / KV_ST) & 1);
+                    okS[j] = s_n[j] < NT_all && c && k;
+                    okP[j] = p_n[j] < NT_all && mbar_test_wait(p_ready + g, p_n[j] & 1);
+                }
+#pragma unroll
+                for (int j = 0; j < NGI; ++j) {
+                    const int g = g0 + j;
+                    if (okP[j]) {  // O(g) += P(g, m) V(g, m)
                         tc_fence_after();
-                        const uint64_t dq = make_desc_sw64(smem_u32(sQ + (g * 2 + (s_il[g] & 1)) * QT_BYTES));
-                        const uint64_t dk = make_desc_sw64(smem_u32(sKV + (g * KV_ST + s_st[g]) * 2 * KT_BYTES));
+                        const uint64_t dv = make_desc_sw64(kvbase + (g * KV_ST + p_st[j]) * 2 * KT_BYTES + KT_BYTES);
+                        const uint32_t tP = tmem + g * 128 + 64, tO = tmem + g * 128 + 96;
+                        if (elect_one()) {
+#pragma unroll
+                            for (int ks = 0; ks < BK / 16; ++ks)
+                                mma_ts(tO, tP + ks * 8, dv + (uint64_t)ks * 64, idescO, (p_kt[j] > 0 || ks > 0) ? 1u : 0u);
+                            mma_commit(kv_free + g * KV_ST + p_st[j]);
+                            mma_commit(pv_done + g);
+                        }
+                        __syncwarp();
+                        ++p_n[j];
+                        --remaining;
+                        if (++p_st[j] == KV_ST) p_st[j] = 0;
+                        if (++p_kt[j] == TPR) p_kt[j] = 0;
+                    }
+                    if (okS[j]) {  // S(g, m): S columns free (tile m-1 read out), K (and Q) of tile m in shared memory
+                        tc_fence_after();
+                        const uint64_t dq = make_desc_sw64(qbase + (g * 2 + s_par[j]) * QT_BYTES);
+                        const uint64_t dk = make_desc_sw64(kvbase + (g * KV_ST + s_st[j]) * 2 * KT_BYTES);
                         const uint32_t tS = tmem + g * 128;
                         if (elect_one()) {
                             mma_ss(tS, dq, dk, idescS, 0);
@@ -171,27 +201,9 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                             mma_commit(s_full + g);
                         }
                         __syncwarp();
-                        ++s_n[g];
-                        if (++s_st[g] == KV_ST) s_st[g] = 0;
-                        if (++s_kt[g] == TPR) { s_kt[g] = 0; ++s_il[g]; }
-                    }
-                    // O(g) += P(g, m) V(g, m)
-                    if (p_n[g] < NT_all && mbar_test_wait(p_ready + g, p_n[g] & 1)) {
-                        tc_fence_after();
-                        const uint64_t dv = make_desc_sw64(smem_u32(sKV + (g * KV_ST + p_st[g]) * 2 * KT_BYTES + KT_BYTES));
-                        const uint32_t tP = tmem + g * 128 + 64, tO = tmem + g * 128 + 96;
-                        if (elect_one()) {
-#pragma unroll
-                            for (int ks = 0; ks < BK / 16; ++ks)
-                                mma_ts(tO, tP + ks * 8, dv + (uint64_t)ks * 64, idescO, (p_kt[g] > 0 || ks > 0) ? 1u : 0u);
-                            mma_commit(kv_free + g * KV_ST + p_st[g]);
-                            mma_commit(pv_done + g);
-                        }
-                        __syncwarp();
-                        ++p_n[g];
-                        --remaining;
-                        if (++p_st[g] == KV_ST) p_st[g] = 0;
-                        if (++p_kt[g] == TPR) p_kt[g] = 0;
+                        ++s_n[j];
+                        if (++s_st[j] == KV_ST) s_st[j] = 0;
+                        if (++s_kt[j] == TPR) { s_kt[j] = 0; s_par[j] ^= 1; }
                     }
                 }
             }
