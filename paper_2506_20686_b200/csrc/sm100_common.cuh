@@ -278,5 +278,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d, int variant, int box_pos);
 // 3-D map over a [BH, N, N] bf16 plane stack, dims (col, row, bh); box = {64, box_rows, 1}, SWIZZLE_128B.
 bool make_tmap_plane(CUtensorMap* out, const void* base, int BH, int N, int box_rows);
+// 3-D map over a [BH, N, N] fp32 plane stack, dims (col, row, bh); box = {32, box_rows, 1} (128-byte rows), SWIZZLE_128B.
+bool make_tmap_plane_f32(CUtensorMap* out, const void* base, int BH, int N, int box_rows);
 
 }  // namespace tri

@@ -26,11 +26,11 @@ namespace {
 constexpr int NG = 4;                      // softmax groups per CTA
 constexpr int BQ = 128, BK = 64, DH = 32;
 constexpr int KV_ST = 3;                   // K/V ring stages per group
-constexpr int NB = 3;                      // bias ring stages (shared by the groups)
+constexpr int NB = 2;                      // bias ring stages (shared by the groups)
 constexpr int QT_BYTES = BQ * DH * 2;      // 8 KB: 128 x 32 bf16
 constexpr int KT_BYTES = BK * DH * 2;      // 4 KB:  64 x 32 bf16
-constexpr int BIAS_BYTES = BQ * BK * 2;    // 16 KB: [128 q][64 k] bf16, SWIZZLE_128B
-constexpr float kLazy = 5.0f;              // lazy-rescale threshold on the running max (natural-log units)
+constexpr int BIAS_BYTES = BQ * BK * 4;    // 32 KB: two [128 q][32 k] fp32 boxes (log2e * bias), SWIZZLE_128B
+constexpr float kLazy = 7.0f;              // lazy-rescale threshold on the running max (log2 units)
 constexpr int FWD_THREADS = (NG + 1) * 128;
 
 struct FwdSmem {
@@ -126,6 +126,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                     if (elect_one()) {
                         mbar_expect_tx(bias_full + bst, BIAS_BYTES);
                         tma_load_3d(sBias + bst * BIAS_BYTES, &tmBias, bias_full + bst, kt * BK, it.q0, bh);
+                        tma_load_3d(sBias + bst * BIAS_BYTES + BIAS_BYTES / 2, &tmBias, bias_full + bst, kt * BK + 32, it.q0, bh);
                     }
                     __syncwarp();
 #pragma unroll 1
@@ -217,8 +218,8 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         const int row = tid & 127;                                  // query row inside the block = TMEM lane
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
         const uint32_t tS = tmem + g * 128 + lane_off, tP = tS + 64, tO = tS + 96;
-        const float scale = rsqrtf((float)DH);
-        const uint64_t scale2 = pack2(scale, scale), l2e2 = pack2(kLog2e, kLog2e);
+        const float sl = rsqrtf((float)DH) * kLog2e;  // scores are kept in log2 units: x = S * scale * log2e + log2e * bias
+        const uint64_t sl2 = pack2(sl, sl);
         const int NW = N / 64;  // mask words per row
         int bst = 0, bph = 0;
         int n = 0;
@@ -242,23 +243,19 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 tmem_ld32(tS, *(uint32_t(*)[32])&raw[0]);
                 tmem_ld32(tS + 32, *(uint32_t(*)[32])&raw[32]);
                 mbar_wait(bias_full + bst, bph);
-                const uint8_t* brow = sBias + bst * BIAS_BYTES + row * 128;
+                const uint8_t* brow = sBias + bst * BIAS_BYTES + row * 128;  // my row in the two 32-column boxes
                 tmem_ld_wait();
                 tc_fence_before();
                 warp_arrive(consumed + g);  // S(n) is in registers: the issuer may overwrite the S columns
 
-                // ---- scores of my query row: x = scale*S + bias (+ mask) ---------------------------------------
+                // ---- scores of my query row in log2 units: x = (scale*log2e)*S + log2e*bias (+ mask) -------------------
                 float x[BK];
 #pragma unroll
-                for (int c8 = 0; c8 < BK / 8; ++c8) {
-                    const uint4 bv = lds128(brow + ((c8 ^ (row & 7)) << 4));
-                    const uint32_t w[4] = {bv.x, bv.y, bv.z, bv.w};
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int c = c8 * 8 + e * 2;
-                        unpack2(fma2(pack2(__uint_as_float(raw[c]), __uint_as_float(raw[c + 1])), scale2,
-                                     pack2(bf16_lo(w[e]), bf16_hi(w[e]))), x[c], x[c + 1]);
-                    }
+                for (int c4 = 0; c4 < BK / 4; ++c4) {
+                    const float4 bv = lds128f(brow + (c4 >> 3) * (BIAS_BYTES / 2) + (((c4 & 7) ^ (row & 7)) << 4));
+                    const int c = c4 * 4;
+                    unpack2(fma2(pack2(__uint_as_float(raw[c]), __uint_as_float(raw[c + 1])), sl2, pack2(bv.x, bv.y)), x[c], x[c + 1]);
+                    unpack2(fma2(pack2(__uint_as_float(raw[c + 2]), __uint_as_float(raw[c + 3])), sl2, pack2(bv.z, bv.w)), x[c + 2], x[c + 3]);
                 }
                 // my generic-proxy reads of the bias tile must be complete before the producer's TMA (async proxy) may
                 // overwrite it: without the proxy fence the arrive can overtake the ld.shared of a busy warp
@@ -287,15 +284,14 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 const bool bump = mx > m_old + kLazy;
                 const float m_new = bump ? mx : m_old;
                 const float m_safe = (m_new == -INFINITY) ? 0.0f : m_new;
-                const float alpha = bump ? ex2((m_old - m_safe) * kLog2e) : 1.0f;
-                const float mneg = -m_safe * kLog2e;
-                const uint64_t mneg2 = pack2(mneg, mneg);
+                const float alpha = bump ? ex2(m_old - m_safe) : 1.0f;
+                const uint64_t mneg2 = pack2(-m_safe, -m_safe);
                 uint64_t lacc4[4] = {pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f)};
                 uint32_t pk[BK / 2];
 #pragma unroll
                 for (int e = 0; e < BK / 2; ++e) {
                     float a0, a1;
-                    unpack2(fma2(pack2(x[2 * e], x[2 * e + 1]), l2e2, mneg2), a0, a1);
+                    unpack2(add2(pack2(x[2 * e], x[2 * e + 1]), mneg2), a0, a1);
                     const float p0 = ex2(a0), p1 = ex2(a1);
                     lacc4[e & 3] = add2(lacc4[e & 3], pack2(p0, p1));
                     pk[e] = pack_bf16(p0, p1);
@@ -347,7 +343,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 op[j] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
             const long long loff = (long long)it.b * N * p.H * N + (long long)it.h * N + (long long)r * p.lR + (long long)(it.q0 + row) * p.lQ;
-            LSE[loff] = l_run > 0.0f ? m_run + __logf(l_run) : -INFINITY;
+            LSE[loff] = l_run > 0.0f ? m_run * kLn2 + __logf(l_run) : -INFINITY;
         }
     }
     tc_fence_before();
@@ -364,6 +360,24 @@ __global__ void transpose_bf16_kernel(const __nv_bfloat16* __restrict__ in, __nv
     __syncthreads();
     const int xo = blockIdx.y * 32 + threadIdx.x, yo0 = blockIdx.x * 32;
     for (int j = threadIdx.y; j < 32; j += 8) out[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
+}
+
+// fp32 planes of f * bias for the softmax warps (no bf16 unpacking in the inner loops): nat[bh][y][x] = f*in[bh][y][x],
+// tr[bh][x][y] = f*in[bh][y][x]; either output may be null.  N^2 H B elements: negligible next to the N^3 work.
+__global__ void bias_planes_kernel(const __nv_bfloat16* __restrict__ in, float* __restrict__ nat, float* __restrict__ tr,
+                                   int N, float f) {
+    __shared__ float tile[32][33];
+    const long long plane = (long long)blockIdx.z * N * N;
+    const int x = blockIdx.x * 32 + threadIdx.x, y0 = blockIdx.y * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) {
+        const float v = f * __bfloat162float(in[plane + (long long)(y0 + j) * N + x]);
+        if (nat) nat[plane + (long long)(y0 + j) * N + x] = v;
+        tile[j][threadIdx.x] = v;
+    }
+    if (!tr) return;
+    __syncthreads();
+    const int xo = blockIdx.y * 32 + threadIdx.x, yo0 = blockIdx.x * 32;
+    for (int j = threadIdx.y; j < 32; j += 8) tr[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
 }
 
 // keep flags [B,N,N] (u8) -> one 64-bit word per (b, row r, 64-key tile): bit k = key 64*w + k of row r is visible.
@@ -397,6 +411,12 @@ tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cuda
     return TRI_OK;
 }
 
+tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int N, float f, cudaStream_t st) {
+    ProfScope ps("bias_planes_kernel", st);
+    bias_planes_kernel<<<dim3(N / 32, N / 32, BH), dim3(32, 8), 0, st>>>((const __nv_bfloat16*)in, nat, tr, N, f);
+    return TRI_OK;
+}
+
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st) {
     ProfScope ps("pack_mask_kernel", st);
     pack_mask_kernel<<<dim3((p.N / 64 + 3) / 4, p.N, p.B), 128, 0, st>>>(mask, (unsigned long long*)bits, p);
@@ -415,7 +435,7 @@ bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && 
 size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.N * (p.N / 64) * 8, 256); }
 
 size_t sm100_fwd_workspace(const Problem& p) {
-    return sm100_maskbits_bytes(p) + (p.variant == TRI_ENDING ? align_up((size_t)p.B * p.H * p.N * p.N * 2, 256) : 0);
+    return sm100_maskbits_bytes(p) + align_up((size_t)p.B * p.H * p.N * p.N * 4, 256);  // + log2e * bias[q][k], fp32
 }
 
 tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void* V, const void* G, const void* bias,
@@ -427,17 +447,17 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
         if (s != TRI_OK) return s;
         TRI_LAUNCH_CHECK("pack_mask_kernel");
     }
-    const void* bias_qk = bias;
-    if (p.variant == TRI_ENDING) {
-        void* biasT = (char*)ws + sm100_maskbits_bytes(p);
-        tri_status s = sm100_transpose_planes(bias, biasT, p.B * p.H, p.N, st);
+    // log2e * bias as fp32 planes in [q][k] order (the ending-node variant reads bias[b,h,k,q]: transposed here)
+    float* biasL = (float*)((char*)ws + sm100_maskbits_bytes(p));
+    {
+        const bool tr = p.variant == TRI_ENDING;
+        tri_status s = sm100_bias_planes(bias, tr ? nullptr : biasL, tr ? biasL : nullptr, p.B * p.H, p.N, kLog2e, st);
         if (s != TRI_OK) return s;
-        TRI_LAUNCH_CHECK("sm100_transpose_bf16");
-        bias_qk = biasT;
+        TRI_LAUNCH_CHECK("bias_planes_kernel");
     }
     CUtensorMap tQ, tK, tV, tB;
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK) ||
-        !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane(&tB, bias_qk, p.B * p.H, p.N, BQ))
+        !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane_f32(&tB, biasL, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
     TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));

@@ -86,6 +86,8 @@ tri_status simt_bwd(const Problem& p, tri_dtype dt, const void* dO, const void* 
 // ---- bf16 tcgen05 / TMA path (sm100_fwd.cu, sm100_bwd.cu) ------------------------------------
 bool sm100_supported(const Problem& p, tri_dtype dt);
 tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cudaStream_t st);  // bf16 [BH,N,N]
+// fp32 planes f*bias: nat (same orientation) and / or tr (transposed); either may be null
+tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int N, float f, cudaStream_t st);
 // keep flags -> one 64-bit word per (b, row, 64-key tile), rows / keys in the variant's sense
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st);
 size_t sm100_maskbits_bytes(const Problem& p);
