@@ -727,8 +727,9 @@ __global__ void __launch_bounds__(256) sm100_dbias_reduce_kernel(const float* __
 // ---- host side ------------------------------------------------------------------------------------------------
 namespace {
 struct BwdWs {
-    size_t d_off, da_off, biast_off, planes_off, total;
-    int G;  // row slices of the dBias kernel
+    size_t d_off, da_off, biast_off, biasl_off, mask_off, planes_off, total;
+    int G;   // row slices of the tile-stationary kernel (dqdb, or the dbias fallback)
+    int C;   // cluster size of the fused dQ + dBias kernel (0: not covered, use dq + dbias)
 };
 // Split the broadcast-row axis of the tile-stationary dBias kernel over G CTAs per tile when the tile grid alone
 // cannot fill the 148 SMs (1 CTA/SM): pick G in 1..8 minimising waves * rows-per-CTA.
@@ -750,9 +751,14 @@ BwdWs bwd_ws_layout(const Problem& p) {
     w.d_off = o; o += align_up((size_t)p.B * p.N * p.H * p.N * sizeof(float), 256);
     w.da_off = o; o += align_up((size_t)p.B * p.N * p.H * p.N * p.d * 2, 256);
     w.biast_off = o; o += align_up((size_t)p.B * p.H * p.N * p.N * 2, 256);
-    w.G = dbias_split(p);
+    w.biasl_off = o; o += align_up((size_t)p.B * p.H * p.N * p.N * 4, 256);
+    w.mask_off = o; o += sm100_maskbits_bytes(p);
+    w.C = sm100_dqdb_cluster(p.N);
+    const int g1 = dbias_split(p), g2 = w.C ? sm100_dqdb_split(p) : 1;
+    w.G = w.C ? g2 : g1;
+    const int gmax = g1 > g2 ? g1 : g2;  // the fallback pair must fit too (device without cluster support)
     w.planes_off = o;
-    if (w.G > 1) o += align_up((size_t)w.G * p.B * p.H * p.N * p.N * sizeof(float), 256);
+    if (gmax > 1) o += align_up((size_t)gmax * p.B * p.H * p.N * p.N * sizeof(float), 256);
     w.total = o;
     return w;
 }
@@ -796,8 +802,6 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
 
     // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
     if ((s = set_smem(sm100_dkdv_kernel<RKV>, DkdvSmem<RKV>::total)) != TRI_OK) return s;
-    if ((s = set_smem(sm100_dq_kernel<RQ>, DqSmem<RQ>::total)) != TRI_OK) return s;
-    if ((s = set_smem(sm100_dbias_kernel, DbiasSmem::total)) != TRI_OK) return s;
     {
         ProfScope ps("sm100_dkdv_kernel", st);
         const unsigned grid = (unsigned)((long long)p.B * (p.N / RKV) * p.H * (p.N / 128));
@@ -805,26 +809,46 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
                                                                        (__nv_bfloat16*)dK, (__nv_bfloat16*)dV);
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
-    {
-        ProfScope ps("sm100_dq_kernel", st);
-        const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
-        sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
-                                                                 (__nv_bfloat16*)dQ);
-    }
-    TRI_LAUNCH_CHECK("sm100_dq_kernel");
     float* planes = (float*)((char*)ws + w.planes_off);
-    {
-        ProfScope ps("sm100_dbias_kernel", st);
-        const unsigned grid = (unsigned)((long long)p.B * p.H * (p.N / 128) * (p.N / 128) * w.G);
-        sm100_dbias_kernel<<<grid, 288, DbiasSmem::total, st>>>(tQ128, tA128, tK128, tV128, tBqk, p, mask, LSE, Dws, dBias,
-                                                                planes, w.G);
+    int Gs = w.G;
+    const int grid2 = w.C ? sm100_dqdb_grid(p, w.C, w.G) : 0;
+    if (grid2 > 0) {
+        // stage 2, fused: dQ and dBias from one recomputation of P / dS (cluster over the key tiles of a query block)
+        unsigned long long* maskbits = nullptr;
+        if (mask) {
+            maskbits = (unsigned long long*)((char*)ws + w.mask_off);
+            if ((s = sm100_pack_mask(p, mask, maskbits, st)) != TRI_OK) return s;
+            TRI_LAUNCH_CHECK("pack_mask_kernel");
+        }
+        float* biasL = (float*)((char*)ws + w.biasl_off);
+        const bool tr = p.variant == TRI_ENDING;
+        if ((s = sm100_bias_planes(bias, tr ? nullptr : biasL, tr ? biasL : nullptr, p.B * p.H, p.N, kLog2e, st)) != TRI_OK) return s;
+        TRI_LAUNCH_CHECK("bias_planes_kernel");
+        if ((s = sm100_dqdb_launch(p, w.C, w.G, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dBias, planes, st)) != TRI_OK) return s;
+    } else {
+        Gs = dbias_split(p);
+        if ((s = set_smem(sm100_dq_kernel<RQ>, DqSmem<RQ>::total)) != TRI_OK) return s;
+        if ((s = set_smem(sm100_dbias_kernel, DbiasSmem::total)) != TRI_OK) return s;
+        {
+            ProfScope ps("sm100_dq_kernel", st);
+            const unsigned grid = (unsigned)((long long)p.B * (p.N / RQ) * p.H * (p.N / 128));
+            sm100_dq_kernel<RQ><<<grid, 256, DqSmem<RQ>::total, st>>>(tQ128, tA128, tK64, tV64, tBqk, p, mask, LSE, Dws,
+                                                                     (__nv_bfloat16*)dQ);
+        }
+        TRI_LAUNCH_CHECK("sm100_dq_kernel");
+        {
+            ProfScope ps("sm100_dbias_kernel", st);
+            const unsigned grid = (unsigned)((long long)p.B * p.H * (p.N / 128) * (p.N / 128) * Gs);
+            sm100_dbias_kernel<<<grid, 288, DbiasSmem::total, st>>>(tQ128, tA128, tK128, tV128, tBqk, p, mask, LSE, Dws, dBias,
+                                                                    planes, Gs);
+        }
+        TRI_LAUNCH_CHECK("sm100_dbias_kernel");
     }
-    TRI_LAUNCH_CHECK("sm100_dbias_kernel");
-    if (w.G > 1) {
+    if (Gs > 1) {
         {
             ProfScope ps("sm100_dbias_reduce_kernel", st);
             sm100_dbias_reduce_kernel<<<dim3(p.N / 32, p.N / 32, p.B * p.H), 256, 0, st>>>(
-                planes, dBias, p.B * p.H, p.N, w.G, p.variant == TRI_ENDING ? 1 : 0);
+                planes, dBias, p.B * p.H, p.N, Gs, p.variant == TRI_ENDING ? 1 : 0);
         }
         TRI_LAUNCH_CHECK("sm100_dbias_reduce_kernel");
     }

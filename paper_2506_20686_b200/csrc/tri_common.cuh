@@ -91,6 +91,13 @@ tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int 
 // keep flags -> one 64-bit word per (b, row, 64-key tile), rows / keys in the variant's sense
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st);
 size_t sm100_maskbits_bytes(const Problem& p);
+// fused dQ + dBias stage (sm100_dqdb.cu): cluster size (0 = shape not covered), row split, persistent grid, launch
+int sm100_dqdb_cluster(int N);
+int sm100_dqdb_split(const Problem& p);
+int sm100_dqdb_grid(const Problem& p, int C, int G);
+tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const void* Q, const void* dA, const void* K,
+                             const void* V, const float* biasL_qk, const unsigned long long* maskbits, const float* LSE,
+                             const float* Dws, void* dQ, float* dBias, float* planes, cudaStream_t st);
 int sm100_sm_count();
 size_t sm100_fwd_workspace(const Problem& p);
 size_t sm100_bwd_workspace(const Problem& p);
