@@ -754,9 +754,8 @@ BwdWs bwd_ws_layout(const Problem& p) {
     w.biasl_off = o; o += align_up((size_t)p.B * p.H * p.N * p.N * 4, 256);
     w.mask_off = o; o += sm100_maskbits_bytes(p);
     w.C = sm100_dqdb_cluster(p.N);
-    const int g1 = dbias_split(p), g2 = w.C ? sm100_dqdb_split(p) : 1;
-    w.G = w.C ? g2 : g1;
-    const int gmax = g1 > g2 ? g1 : g2;  // the fallback pair must fit too (device without cluster support)
+    w.G = dbias_split(p);                         // the fallback pair's split
+    const int gmax = w.C ? kDqdbMaxSplit : w.G;   // the fused kernel picks its split (<= kDqdbMaxSplit) at launch
     w.planes_off = o;
     if (gmax > 1) o += align_up((size_t)gmax * p.B * p.H * p.N * p.N * sizeof(float), 256);
     w.total = o;
@@ -810,9 +809,8 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
     float* planes = (float*)((char*)ws + w.planes_off);
-    int Gs = w.G;
-    const int grid2 = w.C ? sm100_dqdb_grid(p, w.C, w.G) : 0;
-    if (grid2 > 0) {
+    int Gs = w.G, C2 = 0, grid2 = 0;
+    if (w.C && sm100_dqdb_plan(p, &C2, &Gs, &grid2)) {
         // stage 2, fused: dQ and dBias from one recomputation of P / dS (cluster over the key tiles of a query block)
         unsigned long long* maskbits = nullptr;
         if (mask) {
@@ -824,7 +822,7 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
         const bool tr = p.variant == TRI_ENDING;
         if ((s = sm100_bias_planes(bias, tr ? nullptr : biasL, tr ? biasL : nullptr, p.B * p.H, p.N, kLog2e, st)) != TRI_OK) return s;
         TRI_LAUNCH_CHECK("bias_planes_kernel");
-        if ((s = sm100_dqdb_launch(p, w.C, w.G, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dBias, planes, st)) != TRI_OK) return s;
+        if ((s = sm100_dqdb_launch(p, C2, Gs, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dBias, planes, st)) != TRI_OK) return s;
     } else {
         Gs = dbias_split(p);
         if ((s = set_smem(sm100_dq_kernel<RQ>, DqSmem<RQ>::total)) != TRI_OK) return s;

@@ -10,15 +10,17 @@
 //     distributed shared memory (rank c receives the running sum of ranks < c, adds its own, passes it on; the last
 //     rank scales and stores dQ).  No floating-point atomics anywhere; every output is bitwise reproducible.
 //
-// Persistent, warp-specialised CTA of 640 threads:
-//   warps 0-11   three compute groups (128 threads = 128 query rows = 128 TMEM lanes); group g owns key tile g of the
-//                CTA: p = exp2(S*scale*log2e + log2e*bias - LSE*log2e), dS = p (dP - D), dBias += dS (fp32 registers),
-//                dS -> bf16 -> TMEM;
-//   warp 12      TMA producer: per row Q_r, dA_r (128 x 32) and K_r, V_r (192 x 32) into a 2-stage ring; per work item
+// Persistent, warp-specialised CTA of 512 threads:
+//   warps 0-7    two compute groups (128 threads = 128 query rows = 128 TMEM lanes); group g owns key tile g of the CTA
+//                and walks its two 32-key halves per row (S / dP ping-pong in TMEM, so the MMAs of one half run under
+//                the math of the other): p = exp2(S*scale*log2e + log2e*bias - LSE*log2e), dS = p (dP - D),
+//                dBias += dS (fp32 registers), dS -> bf16 -> TMEM;
+//   warp 8       TMA producer: per row Q_r, dA_r (128 x 32) and K_r, V_r (128 x 32) into a 3-stage ring; per work item
 //                the fp32 log2e*bias tiles of the groups;
-//   warp 13      tcgen05.mma issuer: S = Q K^T, dP = dA V^T (SS, M128 N64 K2x16) per group, then dQ += dS K (TS, M128 N32
-//                K4x16) in group order into a double-buffered accumulator;
-//   warps 16-19  dQ reducer: TMEM partial -> registers -> + inbox -> next rank's inbox (st.shared::cluster) or global.
+//   warp 9       tcgen05.mma issuer: S = Q K^T, dP = dA V^T (SS, M128 N32 K2x16) per group and half, then
+//                dQ += dS K (TS, M128 N32 K2x16) in a fixed (half, group) order into a double-buffered accumulator;
+//   warps 12-15  dQ reducer: TMEM partial -> registers -> + inbox -> next rank's inbox (st.async into distributed
+//                shared memory, completion counted on the receiver's mbarrier) or, on the last rank, global memory.
 #include <cuda_runtime.h>
 
 #include "sm100_common.cuh"
@@ -29,16 +31,17 @@ using namespace sm100;
 
 namespace {
 
-constexpr int NGB = 3;                                    // compute groups (64-key tiles) per CTA
-constexpr int BQ = 128, BK = 64, DH = 32;
-constexpr int NST = 2;                                    // operand ring stages (one broadcast row each)
+constexpr int NGB = 2;                                    // compute groups (64-key tiles) per CTA
+constexpr int BQ = 128, BK = 64, BH = 32, DH = 32;        // BH: keys per half tile (one MMA / softmax unit)
+constexpr int NST = 3;                                    // operand ring stages (one broadcast row each)
 constexpr int QT_BYTES = BQ * DH * 2;                     // 8 KB
 constexpr int KT_BYTES = BK * DH * 2;                     // 4 KB
-constexpr int STAGE_BYTES = 2 * QT_BYTES + 2 * NGB * KT_BYTES;  // Q, dA, K[192], V[192] = 40 KB
+constexpr int STAGE_BYTES = 2 * QT_BYTES + 2 * NGB * KT_BYTES;  // Q, dA, K[128], V[128] = 32 KB
 constexpr int BIAS_BYTES = BQ * BK * 4;                   // 32 KB per group: two [128 q][32 k] fp32 boxes, SWIZZLE_128B
 constexpr int INBOX_BYTES = BQ * DH * 4;                  // 16 KB: running dQ sum of the lower ranks
 constexpr int NIN = 2;                                    // inbox ring depth
 constexpr int DQDB_THREADS = (NGB + 2) * 128;
+constexpr int TM_DQ = NGB * 128;                          // TMEM column of the dQ accumulators (2 x 32)
 
 struct DqdbSmem {
     static constexpr int op_off = 0;
@@ -49,11 +52,11 @@ struct DqdbSmem {
     static constexpr int b_free = b_full + NST;           // [NST] MMAs of the row done -> producer
     static constexpr int b_bias_full = b_free + NST;
     static constexpr int b_bias_free = b_bias_full + 1;
-    static constexpr int b_s_full = b_bias_free + 1;      // [NGB] S, dP of the row in TMEM
-    static constexpr int b_ds_ready = b_s_full + NGB;     // [NGB] dS of the row in TMEM
-    static constexpr int b_dq_full = b_ds_ready + NGB;    // [2] partial dQ of the row complete
+    static constexpr int b_s_full = b_bias_free + 1;      // [NGB][2] S, dP of the half in TMEM
+    static constexpr int b_ds_ready = b_s_full + 2 * NGB; // [NGB][2] dS of the half in TMEM
+    static constexpr int b_dq_full = b_ds_ready + 2 * NGB;  // [2] partial dQ of the row complete
     static constexpr int b_dq_free = b_dq_full + 2;       // [2] reducer has it in registers
-    static constexpr int b_in_full = b_dq_free + 2;       // [NIN] lower rank wrote my inbox slot (remote arrivals)
+    static constexpr int b_in_full = b_dq_free + 2;       // [NIN] lower rank's st.async bytes landed in my inbox slot
     static constexpr int b_out_free = b_in_full + NIN;    // [NIN] upper rank read its inbox slot (remote arrivals)
     static constexpr int n_bars = b_out_free + NIN;
     static constexpr int total = bar_off + n_bars * 8 + 16 + 1024;
@@ -78,23 +81,13 @@ __device__ __forceinline__ uint32_t map_to_rank(uint32_t saddr, uint32_t rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
     return r;
 }
-__device__ __forceinline__ void st_cluster_v4(uint32_t addr, float a, float b, float c, float d) {
-    asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+// 16-byte asynchronous store into a peer's shared memory; its bytes are counted on the peer's mbarrier (no fences)
+__device__ __forceinline__ void st_async_v4(uint32_t addr, float a, float b, float c, float d, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"(mbar) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t addr) {  // release at cluster scope: my earlier DSMEM stores
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(addr) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {  // acquire at cluster scope
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2, %3;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity), "r"(0x989680u)
-            : "memory");
-    } while (!ok);
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t addr) {  // credit return: no data is published by it
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(addr) : "memory");
 }
 
 struct Item2 { int b, h, q0, rb; };
@@ -155,9 +148,9 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         for (int i = 0; i < NST; ++i) { mbar_init(full + i, 1); mbar_init(freeb + i, 1); }
         mbar_init(bias_full, 1);
         mbar_init(bias_free, nt * 4);
-        for (int i = 0; i < NGB; ++i) { mbar_init(s_full + i, 1); mbar_init(ds_ready + i, 4); }
+        for (int i = 0; i < 2 * NGB; ++i) { mbar_init(s_full + i, 1); mbar_init(ds_ready + i, 4); }
         for (int i = 0; i < 2; ++i) { mbar_init(dq_full + i, 1); mbar_init(dq_free + i, 4); }
-        for (int i = 0; i < NIN; ++i) { mbar_init(in_full + i, 128); mbar_init(out_free + i, 4); }
+        for (int i = 0; i < NIN; ++i) { mbar_init(in_full + i, 1); mbar_init(out_free + i, 4); }
         fence_barrier_init();
     }
     if (warp == 0) tmem_alloc<512>(tmem_slot);
@@ -201,69 +194,74 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             }
         } else if (warp == NGB * 4 + 1) {
             // ---- MMA issuer (warp-uniform control flow; one elected lane issues and commits) ----
-            constexpr uint32_t idescS = make_idesc(128, BK, false, false);
+            constexpr uint32_t idescS = make_idesc(128, BH, false, false);
             constexpr uint32_t idescO = make_idesc(128, DH, false, true);
             const uint32_t opbase = smem_u32(sOp);
-            auto issue_sdp = [&](int s, int g) {
+            // S, dP of half h of group g for the row staged in s: B operands = rows [32h, 32h+32) of the K / V tiles
+            auto issue_sdp = [&](int s, int g, int h) {
                 const uint32_t st = opbase + s * STAGE_BYTES;
                 const uint64_t dq = make_desc_sw64(st), da = make_desc_sw64(st + QT_BYTES);
-                const uint64_t dk = make_desc_sw64(st + 2 * QT_BYTES + g * KT_BYTES);
-                const uint64_t dv = make_desc_sw64(st + 2 * QT_BYTES + (NGB + g) * KT_BYTES);
-                const uint32_t tS = tmem + g * 128, tDP = tS + 64;
+                const uint64_t dk = make_desc_sw64(st + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2));
+                const uint64_t dv = make_desc_sw64(st + 2 * QT_BYTES + (NGB + g) * KT_BYTES + h * (BH * DH * 2));
+                const uint32_t tS = tmem + g * 128 + h * 64, tDP = tS + 32;
                 if (elect_one()) {
                     mma_ss(tS, dq, dk, idescS, 0);
                     mma_ss(tS, dq + 2, dk + 2, idescS, 1);
                     mma_ss(tDP, da, dv, idescS, 0);
                     mma_ss(tDP, da + 2, dv + 2, idescS, 1);
-                    mma_commit(s_full + g);
+                    mma_commit(s_full + g * 2 + h);
                 }
                 __syncwarp();
             };
             if (NRtot > 0) {
                 mbar_wait(full + 0, 0);
                 tc_fence_after();
-                for (int g = 0; g < nt; ++g) issue_sdp(0, g);
+                for (int h = 0; h < 2; ++h)
+                    for (int g = 0; g < nt; ++g) issue_sdp(0, g, h);
             }
             for (int n = 0; n < NRtot; ++n) {
                 const int s = n % NST, j = n & 1;
-                for (int g = 0; g < nt; ++g) {
-                    mbar_wait(ds_ready + g, n & 1);
-                    if (g == 0 && n >= 2) mbar_wait(dq_free + j, ((n >> 1) - 1) & 1);
-                    tc_fence_after();
-                    const uint64_t dk = make_desc_sw64(opbase + s * STAGE_BYTES + 2 * QT_BYTES + g * KT_BYTES);
-                    const uint32_t tDS = tmem + g * 128 + 64, tDQ = tmem + NGB * 128 + j * 32;
-                    if (elect_one()) {
-#pragma unroll
-                        for (int ks = 0; ks < BK / 16; ++ks)
-                            mma_ts(tDQ, tDS + ks * 8, dk + (uint64_t)ks * 64, idescO, (g > 0 || ks > 0) ? 1u : 0u);
-                        if (g == nt - 1) {
-                            mma_commit(dq_full + j);
-                            mma_commit(freeb + s);
+                for (int h = 0; h < 2; ++h) {
+                    for (int g = 0; g < nt; ++g) {
+                        mbar_wait(ds_ready + g * 2 + h, n & 1);
+                        if (h == 0 && g == 0 && n >= 2) mbar_wait(dq_free + j, ((n >> 1) - 1) & 1);
+                        tc_fence_after();
+                        // dQ_r += dS(g, h) K_r[keys 32h .. 32h+31 of tile g]  (B MN-major: 16 keys = 1024 bytes)
+                        const uint64_t dk = make_desc_sw64(opbase + s * STAGE_BYTES + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2));
+                        const uint32_t tDS = tmem + g * 128 + h * 64 + 32, tDQ = tmem + TM_DQ + j * 32;
+                        if (elect_one()) {
+                            mma_ts(tDQ, tDS, dk, idescO, (h > 0 || g > 0) ? 1u : 0u);
+                            mma_ts(tDQ, tDS + 8, dk + 64, idescO, 1u);
+                            if (h == 1 && g == nt - 1) {
+                                mma_commit(dq_full + j);
+                                mma_commit(freeb + s);
+                            }
                         }
-                    }
-                    __syncwarp();
-                    if (n + 1 < NRtot) {
-                        const int s1 = (n + 1) % NST;
-                        if (g == 0) {
-                            mbar_wait(full + s1, ((n + 1) / NST) & 1);
-                            tc_fence_after();
+                        __syncwarp();
+                        if (n + 1 < NRtot) {
+                            const int s1 = (n + 1) % NST;
+                            if (h == 0 && g == 0) {
+                                mbar_wait(full + s1, ((n + 1) / NST) & 1);
+                                tc_fence_after();
+                            }
+                            issue_sdp(s1, g, h);
                         }
-                        issue_sdp(s1, g);
                     }
                 }
             }
         }
     } else if (warp < NGB * 4) {
         // =============================== compute groups ===============================
-        setmaxnreg_inc<128>();
+        setmaxnreg_inc<208>();
         const int g = warp >> 2;
         if (g < nt) {
             const int row = tid & 127;  // query row inside the block = TMEM lane
             const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-            const uint32_t tS = tmem + g * 128 + lane_off, tDP = tS + 64;
+            const uint32_t tG = tmem + g * 128 + lane_off;
             const float sl = rsqrtf((float)DH) * kLog2e;
             const uint64_t sl2 = pack2(sl, sl);
             const uint8_t* brow = sBias + g * BIAS_BYTES + row * 128;
+            const int sw = row & 7;
             const int tile = t0 + g;
             uint64_t acc2[BK / 2];
 #pragma unroll
@@ -271,59 +269,63 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             int n = 0;
             for (int il = 0; il < n_my; ++il) {
                 const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
-                const long long lbase = (long long)it.b * N * p.H * N + (long long)it.h * N + (long long)(it.q0 + row) * p.lQ;
-                const unsigned long long* mcol = maskbits ? maskbits + ((long long)it.b * N + it.rb) * NW + tile : nullptr;
-                float lse_n = __ldg(LSE + lbase + (long long)it.rb * p.lR), dd_n = __ldg(Dws + lbase + (long long)it.rb * p.lR);
-                uint64_t mb_n = mcol ? ldg_u64(mcol) : ~0ull;
+                const float* lp = LSE + (long long)it.b * N * p.H * N + (long long)it.h * N + (long long)(it.q0 + row) * p.lQ +
+                                  (long long)it.rb * p.lR;
+                const float* dp_ = Dws + (lp - LSE);
+                const unsigned long long* mp = maskbits ? maskbits + ((long long)it.b * N + it.rb) * NW + tile : nullptr;
+                float lse_n = __ldg(lp), dd_n = __ldg(dp_);
+                uint64_t mb_n = mp ? ldg_u64(mp) : ~0ull;
                 mbar_wait(bias_full, il & 1);
                 for (int r = 0; r < NR; ++r, ++n) {
                     const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e;
                     const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd_n, -dd_n);
                     const uint64_t mb = mb_n;
                     if (r + 1 < NR) {
-                        lse_n = __ldg(LSE + lbase + (long long)(it.rb + r + 1) * p.lR);
-                        dd_n = __ldg(Dws + lbase + (long long)(it.rb + r + 1) * p.lR);
-                        if (mcol) mb_n = ldg_u64(mcol + (long long)(r + 1) * NW);
+                        lp += p.lR; dp_ += p.lR;
+                        lse_n = __ldg(lp);
+                        dd_n = __ldg(dp_);
+                        if (mp) { mp += NW; mb_n = ldg_u64(mp); }
                     }
-                    mbar_wait(s_full + g, n & 1);
-                    tc_fence_after();
-                    uint32_t dsb[16];
 #pragma unroll
-                    for (int ch = 0; ch < 4; ++ch) {  // 16 key columns at a time
-                        uint32_t sr[16], dp[16];
-                        tmem_ld16(tS + ch * 16, sr);
-                        tmem_ld16(tDP + ch * 16, dp);
-                        float4 bv[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            bv[i] = lds128f(brow + (ch >> 1) * (BIAS_BYTES / 2) + (((((ch & 1) << 2) + i) ^ (row & 7)) << 4));
+                    for (int h = 0; h < 2; ++h) {
+                        const uint32_t tS = tG + h * 64, tDP = tS + 32;
+                        mbar_wait(s_full + g * 2 + h, n & 1);
+                        tc_fence_after();
+                        uint32_t sr[32], dp[32], dsb[16];
+                        tmem_ld16(tS, sr);
+                        tmem_ld16(tDP, dp);
                         tmem_ld_wait();
+                        tmem_ld16(tS + 16, sr + 16);     // second 16 columns arrive under the math of the first 16
+                        tmem_ld16(tDP + 16, dp + 16);
+                        const uint32_t mh = (uint32_t)(mb >> (h * 32));
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            const float bb[4] = {bv[i].x, bv[i].y, bv[i].z, bv[i].w};
+                        for (int q4 = 0; q4 < 8; ++q4) {  // 4 key columns per step
+                            if (q4 == 4) tmem_ld_wait();
+                            const float4 bv = lds128f(brow + h * (BIAS_BYTES / 2) + ((q4 ^ sw) << 4));
+                            const float bb[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
                             for (int e = 0; e < 2; ++e) {
-                                const int cc = i * 4 + e * 2;  // column inside the chunk
+                                const int cc = q4 * 4 + e * 2;
                                 float x0, x1;
                                 unpack2(fma2(pack2(__uint_as_float(sr[cc]), __uint_as_float(sr[cc + 1])), sl2, pack2(bb[e * 2], bb[e * 2 + 1])), x0, x1);
-                                if (mb != ~0ull) {
-                                    if (!((mb >> (ch * 16 + cc)) & 1ull)) x0 = -INFINITY;
-                                    if (!((mb >> (ch * 16 + cc + 1)) & 1ull)) x1 = -INFINITY;
+                                if (mh != 0xffffffffu) {
+                                    if (!((mh >> cc) & 1u)) x0 = -INFINITY;
+                                    if (!((mh >> (cc + 1)) & 1u)) x1 = -INFINITY;
                                 }
                                 float a0, a1, s0, s1;
                                 unpack2(add2(pack2(x0, x1), nl2), a0, a1);
                                 const uint64_t p2 = pack2(ex2(a0), ex2(a1));
                                 const uint64_t ds2 = mul2(p2, add2(pack2(__uint_as_float(dp[cc]), __uint_as_float(dp[cc + 1])), nd2));
-                                acc2[ch * 8 + (cc >> 1)] = add2(acc2[ch * 8 + (cc >> 1)], ds2);
+                                acc2[h * 16 + (cc >> 1)] = add2(acc2[h * 16 + (cc >> 1)], ds2);
                                 unpack2(ds2, s0, s1);
-                                dsb[(ch & 1) * 8 + (cc >> 1)] = pack_bf16(s0, s1);
+                                dsb[cc >> 1] = pack_bf16(s0, s1);
                             }
                         }
-                        if (ch & 1) tmem_st16(tDP + (ch >> 1) * 16, dsb);  // dS (bf16 pairs) over the dP columns already read
+                        tmem_st16(tDP, dsb);  // dS (bf16 pairs) over the dP columns already read
+                        tmem_st_wait();
+                        tc_fence_before();
+                        warp_arrive(ds_ready + g * 2 + h);
                     }
-                    tmem_st_wait();
-                    tc_fence_before();
-                    warp_arrive(ds_ready + g);
                 }
                 // ---- item done: my 64 dBias values of query row q0+row (level-1 sum over rows rb..rb+NR-1, ascending) ----
                 float acc[BK];
@@ -356,21 +358,24 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         // =============================== dQ reducer warpgroup ===============================
         setmaxnreg_dec<56>();
         const int row = tid & 127;
+        const int sw = row & 7;
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
         const float scale = rsqrtf((float)DH);
-        const uint32_t inbox_local = smem_u32(sInbox);
-        const uint32_t inbox_next = (c + 1 < C) ? map_to_rank(inbox_local, (uint32_t)(c + 1)) : 0u;
+        const uint32_t inbox_next = (c + 1 < C) ? map_to_rank(smem_u32(sInbox), (uint32_t)(c + 1)) : 0u;
         const uint32_t infull_next = (c + 1 < C) ? map_to_rank(smem_u32(in_full), (uint32_t)(c + 1)) : 0u;
         const uint32_t outfree_prev = (c > 0) ? map_to_rank(smem_u32(out_free), (uint32_t)(c - 1)) : 0u;
+        if (c > 0 && tid == (NGB + 1) * 128)  // arm both inbox slots for their first use
+            for (int i = 0; i < NIN && i < NRtot; ++i) mbar_expect_tx(in_full + i, INBOX_BYTES);
         int n = 0;
         for (int il = 0; il < n_my; ++il) {
             const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
-            for (int r = 0; r < NR; ++r, ++n) {
+            __nv_bfloat16* qp = dQ + (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)it.rb * p.sSlice + (long long)(it.q0 + row) * p.sPos;
+            for (int r = 0; r < NR; ++r, ++n, qp += p.sSlice) {
                 const int j = n & 1, ph = (n >> 1) & 1;
                 mbar_wait(dq_full + j, ph);
                 tc_fence_after();
                 uint32_t v[32];
-                tmem_ld32(tmem + NGB * 128 + j * 32 + lane_off, v);
+                tmem_ld32(tmem + TM_DQ + j * 32 + lane_off, v);
                 tmem_ld_wait();
                 tc_fence_before();
                 warp_arrive(dq_free + j);
@@ -378,28 +383,27 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 #pragma unroll
                 for (int i = 0; i < 32; ++i) f[i] = __uint_as_float(v[i]);
                 if (c > 0) {  // running sum of ranks 0..c-1 (fixed order: deterministic)
-                    mbar_wait_cluster(in_full + j, ph);
+                    mbar_wait(in_full + j, ph);
                     const uint8_t* src = sInbox + j * INBOX_BYTES + row * 128;
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
-                        const float4 t = lds128f(src + ((i ^ (row & 7)) << 4));
+                        const float4 t = lds128f(src + ((i ^ sw) << 4));
                         f[4 * i] = t.x + f[4 * i]; f[4 * i + 1] = t.y + f[4 * i + 1];
                         f[4 * i + 2] = t.z + f[4 * i + 2]; f[4 * i + 3] = t.w + f[4 * i + 3];
                     }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_remote(outfree_prev + j * 8);  // the slot may be rewritten
+                    // all 128 readers are done with the slot: re-arm it for row n + NIN, then hand the credit back
+                    named_bar_sync(1, 128);
+                    if (tid == (NGB + 1) * 128 && n + NIN < NRtot) mbar_expect_tx(in_full + j, INBOX_BYTES);
+                    if (lane == 0) mbar_arrive_remote(outfree_prev + j * 8);
                 }
                 if (c + 1 < C) {
-                    if (n >= NIN) mbar_wait_cluster(out_free + j, (ph ^ 1));
+                    if (n >= NIN) mbar_wait(out_free + j, ph ^ 1);
                     const uint32_t dst = inbox_next + j * INBOX_BYTES + row * 128;
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
-                        st_cluster_v4(dst + ((i ^ (row & 7)) << 4), f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
-                    mbar_arrive_remote(infull_next + j * 8);
+                        st_async_v4(dst + ((i ^ sw) << 4), f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3], infull_next + j * 8);
                 } else {  // last rank: dQ = scale * sum
-                    const long long off = (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)(it.rb + r) * p.sSlice +
-                                          (long long)(it.q0 + row) * p.sPos;
-                    uint4* pq = (uint4*)(dQ + off);
+                    uint4* pq = (uint4*)qp;
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         uint32_t a[4];
@@ -428,29 +432,14 @@ int sm100_dqdb_cluster(int N) {
     return 0;
 }
 
-// Row slices per (b, h, query block): device-independent (the workspace size depends on it), assuming 148 / C resident
-// clusters; minimises waves * rows per item.
-int sm100_dqdb_split(const Problem& p) {
+// Launch plan on the current device: cluster size C, row slices G per (b, h, query block) (<= kDqdbMaxSplit, chosen to
+// minimise waves * rows per item for the number of clusters the device can hold), persistent grid (a multiple of C).
+// Returns false if the kernel cannot run on this device / shape.
+bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
     const int C = sm100_dqdb_cluster(p.N);
-    if (C == 0) return 1;
-    const int ncl = 148 / C;
-    const long long base = (long long)p.B * p.H * (p.N / BQ);
-    int bestG = 1;
-    double best = 1e30;
-    for (int G = 1; G <= 8; ++G) {
-        if (p.N % G) continue;
-        const double waves = (double)((base * G + ncl - 1) / ncl);
-        const double cost = waves * (p.N / G + 16);
-        if (cost < best * 0.98) { best = cost; bestG = G; }
-    }
-    return bestG;
-}
-
-// persistent grid (a multiple of the cluster size C), 0 if the kernel cannot run on this device / shape
-int sm100_dqdb_grid(const Problem& p, int C, int G) {
-    if (C == 0) return 0;
-    if (cudaFuncSetAttribute(sm100_dqdb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DqdbSmem::total) != cudaSuccess) return 0;
-    if (C > 8 && cudaFuncSetAttribute(sm100_dqdb_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return 0;
+    if (C == 0) return false;
+    if (cudaFuncSetAttribute(sm100_dqdb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DqdbSmem::total) != cudaSuccess) return false;
+    if (C > 8 && cudaFuncSetAttribute(sm100_dqdb_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return false;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(C * 64));
     cfg.blockDim = dim3(DQDB_THREADS);
@@ -462,10 +451,21 @@ int sm100_dqdb_grid(const Problem& p, int C, int G) {
     int ncl = 0;
     if (cudaOccupancyMaxActiveClusters(&ncl, sm100_dqdb_kernel, &cfg) != cudaSuccess || ncl <= 0) {
         cudaGetLastError();
-        return 0;
+        return false;
     }
-    const long long items = (long long)p.B * p.H * (p.N / BQ) * G;
-    return (int)((items < ncl ? items : ncl) * C);
+    const long long base = (long long)p.B * p.H * (p.N / BQ);
+    int bestG = 1;
+    double best = 1e30;
+    for (int G = 1; G <= kDqdbMaxSplit; ++G) {
+        if (p.N % G) continue;
+        const double waves = (double)((base * G + ncl - 1) / ncl);
+        const double cost = waves * (p.N / G + 12);  // + per-item fill / drain / dBias flush in row units
+        if (cost < best * 0.99) { best = cost; bestG = G; }
+    }
+    const long long items = base * bestG;
+    *Cout = C; *Gout = bestG;
+    *grid = (int)((items < ncl ? items : ncl) * C);
+    return true;
 }
 
 tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const void* Q, const void* dA, const void* K, const void* V,

@@ -93,8 +93,8 @@ tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bi
 size_t sm100_maskbits_bytes(const Problem& p);
 // fused dQ + dBias stage (sm100_dqdb.cu): cluster size (0 = shape not covered), row split, persistent grid, launch
 int sm100_dqdb_cluster(int N);
-int sm100_dqdb_split(const Problem& p);
-int sm100_dqdb_grid(const Problem& p, int C, int G);
+constexpr int kDqdbMaxSplit = 8;  // the workspace holds this many partial dBias planes
+bool sm100_dqdb_plan(const Problem& p, int* C, int* G, int* grid);
 tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const void* Q, const void* dA, const void* K,
                              const void* V, const float* biasL_qk, const unsigned long long* maskbits, const float* LSE,
                              const float* Dws, void* dQ, float* dBias, float* planes, cudaStream_t st);
