@@ -11,16 +11,20 @@
 //     rank scales and stores dQ).  No floating-point atomics anywhere; every output is bitwise reproducible.
 //
 // Persistent, warp-specialised CTA of 512 threads:
-//   warps 0-7    two compute groups (128 threads = 128 query rows = 128 TMEM lanes); group g owns key tile g of the CTA
-//                and walks its two 32-key halves per row (S / dP ping-pong in TMEM, so the MMAs of one half run under
-//                the math of the other): p = exp2(S*scale*log2e + log2e*bias - LSE*log2e), dS = p (dP - D),
-//                dBias += dS (fp32 registers), dS -> bf16 -> TMEM;
+//   warps 0-7    two compute groups (128 threads = 128 query rows = 128 TMEM lanes); group g owns key tile g of the CTA,
+//                keeps its fp32 log2e*bias tile and its dBias tile in REGISTERS for the whole work item, and walks the two
+//                32-key halves of the tile per row (S / dP ping-pong in TMEM, so the MMAs of one half run under the math
+//                of the other): p = exp2(S*scale*log2e + log2e*bias - LSE*log2e), dS = p (dP - D), dBias += dS,
+//                dS -> bf16 -> TMEM;
 //   warp 8       TMA producer: per row Q_r, dA_r (128 x 32) and K_r, V_r (128 x 32) into a 3-stage ring; per work item
-//                the fp32 log2e*bias tiles of the groups;
-//   warp 9       tcgen05.mma issuer: S = Q K^T, dP = dA V^T (SS, M128 N32 K2x16) per group and half, then
-//                dQ += dS K (TS, M128 N32 K2x16) in a fixed (half, group) order into a double-buffered accumulator;
-//   warps 12-15  dQ reducer: TMEM partial -> registers -> + inbox -> next rank's inbox (st.async into distributed
-//                shared memory, completion counted on the receiver's mbarrier) or, on the last rank, global memory.
+//                the bias tiles of the groups;
+//   warp 9       S / dP issuer: per row, Q_r and dA_r go shared memory -> TMEM once (tcgen05.cp), so the eight
+//                S = Q K^T, dP = dA V^T MMAs of the row (per group and half, TS form) only read their 32-key B operands
+//                from shared memory;
+//   warp 10      dQ issuer: dQ += dS K (TS, M128 N32 K2x16) in a fixed (half, group) order into a double-buffered
+//                accumulator;
+//   warps 12-15  dQ reducer: partial dQ of a row: TMEM -> registers -> + inbox -> next rank's inbox (st.async into
+//                distributed shared memory, completion counted on the receiver's mbarrier) or, on the last rank, global.
 #include <cuda_runtime.h>
 
 #include "sm100_common.cuh"
@@ -41,20 +45,25 @@ constexpr int BIAS_BYTES = BQ * BK * 4;                   // 32 KB per group: tw
 constexpr int INBOX_BYTES = BQ * DH * 4;                  // 16 KB: running dQ sum of the lower ranks
 constexpr int NIN = 2;                                    // inbox ring depth
 constexpr int DQDB_THREADS = (NGB + 2) * 128;
-constexpr int TM_DQ = NGB * 128;                          // TMEM column of the dQ accumulators (2 x 32)
+// TMEM columns: group g at 160 g: half h at +80 h: S [0,32) | dP [32,64) | dS bf16 [64,80)
+constexpr int TM_GROUP = 160, TM_HALF = 80;
+constexpr int TM_DQ = NGB * TM_GROUP;                     // two 32-column dQ accumulators
+constexpr int TM_QA = TM_DQ + 64;                         // two buffers of Q bf16 [0,16) | dA bf16 [16,32)
 
 struct DqdbSmem {
     static constexpr int op_off = 0;
     static constexpr int bias_off = op_off + NST * STAGE_BYTES;
     static constexpr int inbox_off = bias_off + NGB * BIAS_BYTES;
     static constexpr int bar_off = inbox_off + NIN * INBOX_BYTES;
-    static constexpr int b_full = 0;                      // [NST] TMA -> issuer
+    static constexpr int b_full = 0;                      // [NST] TMA -> issuer, stager
     static constexpr int b_free = b_full + NST;           // [NST] MMAs of the row done -> producer
     static constexpr int b_bias_full = b_free + NST;
     static constexpr int b_bias_free = b_bias_full + 1;
     static constexpr int b_s_full = b_bias_free + 1;      // [NGB][2] S, dP of the half in TMEM
-    static constexpr int b_ds_ready = b_s_full + 2 * NGB; // [NGB][2] dS of the half in TMEM
-    static constexpr int b_dq_full = b_ds_ready + 2 * NGB;  // [2] partial dQ of the row complete
+    static constexpr int b_consumed = b_s_full + 2 * NGB; // [NGB][2] S, dP of the half are in registers
+    static constexpr int b_ds_ready = b_consumed + 2 * NGB;  // [NGB][2] dS of the half in TMEM
+    static constexpr int b_ds_free = b_ds_ready + 2 * NGB;   // [NGB][2] dQ MMAs of the half have read dS
+    static constexpr int b_dq_full = b_ds_free + 2 * NGB; // [2] partial dQ of the row complete
     static constexpr int b_dq_free = b_dq_full + 2;       // [2] reducer has it in registers
     static constexpr int b_in_full = b_dq_free + 2;       // [NIN] lower rank's st.async bytes landed in my inbox slot
     static constexpr int b_out_free = b_in_full + NIN;    // [NIN] upper rank read its inbox slot (remote arrivals)
@@ -123,7 +132,9 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     uint64_t* bias_full = bars + L::b_bias_full;
     uint64_t* bias_free = bars + L::b_bias_free;
     uint64_t* s_full = bars + L::b_s_full;
+    uint64_t* consumed = bars + L::b_consumed;
     uint64_t* ds_ready = bars + L::b_ds_ready;
+    uint64_t* ds_free = bars + L::b_ds_free;
     uint64_t* dq_full = bars + L::b_dq_full;
     uint64_t* dq_free = bars + L::b_dq_free;
     uint64_t* in_full = bars + L::b_in_full;
@@ -148,7 +159,9 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         for (int i = 0; i < NST; ++i) { mbar_init(full + i, 1); mbar_init(freeb + i, 1); }
         mbar_init(bias_full, 1);
         mbar_init(bias_free, nt * 4);
-        for (int i = 0; i < 2 * NGB; ++i) { mbar_init(s_full + i, 1); mbar_init(ds_ready + i, 4); }
+        for (int i = 0; i < 2 * NGB; ++i) {
+            mbar_init(s_full + i, 1); mbar_init(consumed + i, 4); mbar_init(ds_ready + i, 4); mbar_init(ds_free + i, 1);
+        }
         for (int i = 0; i < 2; ++i) { mbar_init(dq_full + i, 1); mbar_init(dq_free + i, 4); }
         for (int i = 0; i < NIN; ++i) { mbar_init(in_full + i, 1); mbar_init(out_free + i, 4); }
         fence_barrier_init();
@@ -193,77 +206,100 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                 }
             }
         } else if (warp == NGB * 4 + 1) {
-            // ---- MMA issuer (warp-uniform control flow; one elected lane issues and commits) ----
-            constexpr uint32_t idescS = make_idesc(128, BH, false, false);
-            constexpr uint32_t idescO = make_idesc(128, DH, false, true);
+            // ---- S / dP issuer (warp-uniform control flow; one elected lane issues and commits) ----
+            // Q_r, dA_r of a row go shared memory -> TMEM once (tcgen05.cp, two rows ahead); a half gets its next S, dP as
+            // soon as the compute group has the previous row's values of that half in registers.  tcgen05.cp / .mma of
+            // one thread execute in issue order, so the copies need no barrier of their own.
+            constexpr uint32_t idesc = make_idesc(128, BH, false, false);  // B = K / V rows, K-major
             const uint32_t opbase = smem_u32(sOp);
-            // S, dP of half h of group g for the row staged in s: B operands = rows [32h, 32h+32) of the K / V tiles
-            auto issue_sdp = [&](int s, int g, int h) {
+            auto stage_qa = [&](int m, int s) {
+                mbar_wait(full + s, (m / NST) & 1);
+                tc_fence_after();
                 const uint32_t st = opbase + s * STAGE_BYTES;
                 const uint64_t dq = make_desc_sw64(st), da = make_desc_sw64(st + QT_BYTES);
-                const uint64_t dk = make_desc_sw64(st + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2));
-                const uint64_t dv = make_desc_sw64(st + 2 * QT_BYTES + (NGB + g) * KT_BYTES + h * (BH * DH * 2));
-                const uint32_t tS = tmem + g * 128 + h * 64, tDP = tS + 32;
+                const uint32_t tQ = tmem + TM_QA + (m & 1) * 32;
                 if (elect_one()) {
-                    mma_ss(tS, dq, dk, idescS, 0);
-                    mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-                    mma_ss(tDP, da, dv, idescS, 0);
-                    mma_ss(tDP, da + 2, dv + 2, idescS, 1);
+                    tmem_cp_128x256b(tQ, dq);
+                    tmem_cp_128x256b(tQ + 8, dq + 2);
+                    tmem_cp_128x256b(tQ + 16, da);
+                    tmem_cp_128x256b(tQ + 24, da + 2);
+                }
+                __syncwarp();
+            };
+            auto issue_sdp = [&](int n, int s, int g, int h) {
+                const uint32_t st = opbase + s * STAGE_BYTES + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2);
+                const uint64_t dk = make_desc_sw64(st), dv = make_desc_sw64(st + NGB * KT_BYTES);
+                const uint32_t tS = tmem + g * TM_GROUP + h * TM_HALF, tDP = tS + 32;
+                const uint32_t tQ = tmem + TM_QA + (n & 1) * 32, tA = tQ + 16;
+                if (elect_one()) {
+                    mma_ts(tS, tQ, dk, idesc, 0);
+                    mma_ts(tS, tQ + 8, dk + 2, idesc, 1);
+                    mma_ts(tDP, tA, dv, idesc, 0);
+                    mma_ts(tDP, tA + 8, dv + 2, idesc, 1);
                     mma_commit(s_full + g * 2 + h);
                 }
                 __syncwarp();
             };
-            if (NRtot > 0) {
-                mbar_wait(full + 0, 0);
-                tc_fence_after();
-                for (int h = 0; h < 2; ++h)
-                    for (int g = 0; g < nt; ++g) issue_sdp(0, g, h);
-            }
+            if (NRtot > 0) stage_qa(0, 0);
+            if (NRtot > 1) stage_qa(1, 1);
+            int s = 0, s2 = 2 % NST;  // ring stages of row n and row n + 2
             for (int n = 0; n < NRtot; ++n) {
-                const int s = n % NST, j = n & 1;
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < 2; ++h)
                     for (int g = 0; g < nt; ++g) {
+                        if (n > 0) {
+                            mbar_wait(consumed + g * 2 + h, (n - 1) & 1);
+                            tc_fence_after();
+                        }
+                        issue_sdp(n, s, g, h);
+                    }
+                if (n + 2 < NRtot) stage_qa(n + 2, s2);  // into the buffer the MMAs just issued read (in-order pipe)
+                if (++s == NST) s = 0;
+                if (++s2 == NST) s2 = 0;
+            }
+        } else if (warp == NGB * 4 + 2) {
+            // ---- dQ issuer: dQ_r += dS(g, h) K_r[keys 32h .. 32h+31 of tile g], strictly in (row, half, group) order ----
+            constexpr uint32_t idescO = make_idesc(128, DH, false, true);  // B = K rows as [key][d], MN-major
+            const uint32_t opbase = smem_u32(sOp);
+            int s = 0;
+            for (int n = 0; n < NRtot; ++n) {
+                const int j = n & 1;
+                for (int h = 0; h < 2; ++h)
+                    for (int g = 0; g < nt; ++g) {
+                        const bool first = h == 0 && g == 0, last = h == 1 && g == nt - 1;
                         mbar_wait(ds_ready + g * 2 + h, n & 1);
-                        if (h == 0 && g == 0 && n >= 2) mbar_wait(dq_free + j, ((n >> 1) - 1) & 1);
+                        if (first && n >= 2) mbar_wait(dq_free + j, ((n >> 1) - 1) & 1);
                         tc_fence_after();
-                        // dQ_r += dS(g, h) K_r[keys 32h .. 32h+31 of tile g]  (B MN-major: 16 keys = 1024 bytes)
+                        // 16 keys of the MN-major B operand = 1024 bytes
                         const uint64_t dk = make_desc_sw64(opbase + s * STAGE_BYTES + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2));
-                        const uint32_t tDS = tmem + g * 128 + h * 64 + 32, tDQ = tmem + TM_DQ + j * 32;
+                        const uint32_t tDS = tmem + g * TM_GROUP + h * TM_HALF + 64, tDQ = tmem + TM_DQ + j * 32;
                         if (elect_one()) {
-                            mma_ts(tDQ, tDS, dk, idescO, (h > 0 || g > 0) ? 1u : 0u);
+                            mma_ts(tDQ, tDS, dk, idescO, first ? 0u : 1u);
                             mma_ts(tDQ, tDS + 8, dk + 64, idescO, 1u);
-                            if (h == 1 && g == nt - 1) {
+                            mma_commit(ds_free + g * 2 + h);
+                            if (last) {
                                 mma_commit(dq_full + j);
-                                mma_commit(freeb + s);
+                                mma_commit(freeb + s);  // S / dP MMAs and copies of the row completed before its dS existed
                             }
                         }
                         __syncwarp();
-                        if (n + 1 < NRtot) {
-                            const int s1 = (n + 1) % NST;
-                            if (h == 0 && g == 0) {
-                                mbar_wait(full + s1, ((n + 1) / NST) & 1);
-                                tc_fence_after();
-                            }
-                            issue_sdp(s1, g, h);
-                        }
                     }
-                }
+                if (++s == NST) s = 0;
             }
         }
     } else if (warp < NGB * 4) {
         // =============================== compute groups ===============================
-        setmaxnreg_inc<208>();
+        setmaxnreg_inc<200>();
         const int g = warp >> 2;
         if (g < nt) {
             const int row = tid & 127;  // query row inside the block = TMEM lane
             const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-            const uint32_t tG = tmem + g * 128 + lane_off;
+            const uint32_t tG = tmem + g * TM_GROUP + lane_off;
             const float sl = rsqrtf((float)DH) * kLog2e;
             const uint64_t sl2 = pack2(sl, sl);
             const uint8_t* brow = sBias + g * BIAS_BYTES + row * 128;
             const int sw = row & 7;
             const int tile = t0 + g;
-            uint64_t acc2[BK / 2];
+            uint64_t acc2[BK / 2], bias2[BK / 2];
 #pragma unroll
             for (int i = 0; i < BK / 2; ++i) acc2[i] = pack2(0.0f, 0.0f);
             int n = 0;
@@ -275,7 +311,16 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                 const unsigned long long* mp = maskbits ? maskbits + ((long long)it.b * N + it.rb) * NW + tile : nullptr;
                 float lse_n = __ldg(lp), dd_n = __ldg(dp_);
                 uint64_t mb_n = mp ? ldg_u64(mp) : ~0ull;
+                // my row of the bias tile -> registers for the whole item; the shared buffer goes back to the producer
                 mbar_wait(bias_full, il & 1);
+#pragma unroll
+                for (int q4 = 0; q4 < 16; ++q4) {
+                    const float4 bv = lds128f(brow + (q4 >> 3) * (BIAS_BYTES / 2) + (((q4 & 7) ^ sw) << 4));
+                    bias2[q4 * 2] = pack2(bv.x, bv.y);
+                    bias2[q4 * 2 + 1] = pack2(bv.z, bv.w);
+                }
+                fence_proxy_async();  // my generic-proxy reads are complete before the producer's TMA may overwrite the tile
+                warp_arrive(bias_free);
                 for (int r = 0; r < NR; ++r, ++n) {
                     const float nl = lse_n == -INFINITY ? -INFINITY : -lse_n * kLog2e;
                     const uint64_t nl2 = pack2(nl, nl), nd2 = pack2(-dd_n, -dd_n);
@@ -288,26 +333,25 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     }
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        const uint32_t tS = tG + h * 64, tDP = tS + 32;
+                        const uint32_t tS = tG + h * TM_HALF, tDP = tS + 32, tDS = tS + 64;
+                        const uint32_t mh = (uint32_t)(mb >> (h * 32));
                         mbar_wait(s_full + g * 2 + h, n & 1);
                         tc_fence_after();
-                        uint32_t sr[32], dp[32], dsb[16];
-                        tmem_ld16(tS, sr);
-                        tmem_ld16(tDP, dp);
-                        tmem_ld_wait();
-                        tmem_ld16(tS + 16, sr + 16);     // second 16 columns arrive under the math of the first 16
-                        tmem_ld16(tDP + 16, dp + 16);
-                        const uint32_t mh = (uint32_t)(mb >> (h * 32));
 #pragma unroll
-                        for (int q4 = 0; q4 < 8; ++q4) {  // 4 key columns per step
-                            if (q4 == 4) tmem_ld_wait();
-                            const float4 bv = lds128f(brow + h * (BIAS_BYTES / 2) + ((q4 ^ sw) << 4));
-                            const float bb[4] = {bv.x, bv.y, bv.z, bv.w};
+                        for (int ch = 0; ch < 2; ++ch) {  // 16 key columns at a time
+                            uint32_t sr[16], dp[16], dsb[8];
+                            tmem_ld16(tS + ch * 16, sr);
+                            tmem_ld16(tDP + ch * 16, dp);
+                            tmem_ld_wait();
+                            if (ch == 1) {  // S, dP of this half are in registers: the issuer may overwrite the columns
+                                tc_fence_before();
+                                warp_arrive(consumed + g * 2 + h);
+                            }
 #pragma unroll
-                            for (int e = 0; e < 2; ++e) {
-                                const int cc = q4 * 4 + e * 2;
+                            for (int e = 0; e < 8; ++e) {
+                                const int cc = ch * 16 + e * 2;  // key column inside the half
                                 float x0, x1;
-                                unpack2(fma2(pack2(__uint_as_float(sr[cc]), __uint_as_float(sr[cc + 1])), sl2, pack2(bb[e * 2], bb[e * 2 + 1])), x0, x1);
+                                unpack2(fma2(pack2(__uint_as_float(sr[e * 2]), __uint_as_float(sr[e * 2 + 1])), sl2, bias2[h * 16 + (cc >> 1)]), x0, x1);
                                 if (mh != 0xffffffffu) {
                                     if (!((mh >> cc) & 1u)) x0 = -INFINITY;
                                     if (!((mh >> (cc + 1)) & 1u)) x1 = -INFINITY;
@@ -315,13 +359,17 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                                 float a0, a1, s0, s1;
                                 unpack2(add2(pack2(x0, x1), nl2), a0, a1);
                                 const uint64_t p2 = pack2(ex2(a0), ex2(a1));
-                                const uint64_t ds2 = mul2(p2, add2(pack2(__uint_as_float(dp[cc]), __uint_as_float(dp[cc + 1])), nd2));
+                                const uint64_t ds2 = mul2(p2, add2(pack2(__uint_as_float(dp[e * 2]), __uint_as_float(dp[e * 2 + 1])), nd2));
                                 acc2[h * 16 + (cc >> 1)] = add2(acc2[h * 16 + (cc >> 1)], ds2);
                                 unpack2(ds2, s0, s1);
-                                dsb[cc >> 1] = pack_bf16(s0, s1);
+                                dsb[e] = pack_bf16(s0, s1);
                             }
+                            if (ch == 0 && n > 0) {  // the dQ MMAs of the previous row have read this half's dS columns
+                                mbar_wait(ds_free + g * 2 + h, (n - 1) & 1);
+                                tc_fence_after();
+                            }
+                            tmem_st8(tDS + ch * 8, dsb);
                         }
-                        tmem_st16(tDP, dsb);  // dS (bf16 pairs) over the dP columns already read
                         tmem_st_wait();
                         tc_fence_before();
                         warp_arrive(ds_ready + g * 2 + h);
@@ -349,14 +397,11 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                         for (int i = 0; i < BK; ++i) out[(long long)i * p.bK] = acc[i];
                     }
                 }
-                // my generic-proxy reads of the bias tiles are complete before the producer's TMA may overwrite them
-                fence_proxy_async();
-                warp_arrive(bias_free);
             }
         }
     } else {
         // =============================== dQ reducer warpgroup ===============================
-        setmaxnreg_dec<56>();
+        setmaxnreg_dec<72>();
         const int row = tid & 127;
         const int sw = row & 7;
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
