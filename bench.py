@@ -10,7 +10,10 @@ matmuls of 2*N^2*d each per (b,row,h)).
 
 Prints ONE JSON line (rank 0).  `value` = model TFLOP/s with inputs resident in HBM; `e2e` = the same
 metric through tri_attn_step_host with pinned HOST buffers (H2D + D2H inside the timed region);
-`roofline` = dominant kernel's model FLOP / its CUDA-event duration against the measured bf16 peak;
+`roofline` = the dominant kernel's EXECUTED tensor FLOP per launch (KERNEL_FLOP_UNITS: every matmul the
+kernel really issues, recomputation included) / its CUDA-event duration against the measured bf16 peak,
+with the MUFU (exp) co-roofline beside it; per-kernel times come from a second, separately profiled loop
+(no events inside the headline timed region); `also` = the N=384 half of the metric (cfg3s / cfg3e);
 `cpu_baseline` = the fp64 oracle timed on this box's host cores on a bounded sample of the workload.
 Multi-GPU (torchrun): rows are independent problems -> each rank runs its own batch, no data-path
 collective (weak scaling); time = max over ranks.
@@ -210,20 +213,19 @@ def aggregate_value(cfg, world: int, ms_step: float) -> float:
 # our arm
 # ------------------------------------------------------------------------------------------------
 # executed tensor FLOP per logit-pass of each kernel, in units of B*H*N^3*d (2 per matmul)
-KERNEL_FLOP_UNITS = (("fwd", 4.0), ("dkdv", 8.0), ("dq", 6.0), ("dbias", 4.0))
+KERNEL_FLOP_UNITS = (("fwd", 4.0), ("dkdv", 8.0), ("dqdb", 6.0), ("dq_", 6.0), ("dbias_kernel", 4.0))
+# one exp per logit and kernel pass: 16 MUFU.EX2 / clk / SM
+KERNEL_EXP_PASSES = (("fwd", 1.0), ("dkdv", 1.0), ("dqdb", 1.0), ("dq_", 1.0), ("dbias_kernel", 1.0))
+# bench.py never reads a stored DRAM-traffic number: `traffic` is null here and the ncu --set full summary of the
+# same commit (dram__bytes_read.sum + dram__bytes_write.sum per launch) is named in `traffic_source`
+TRAFFIC_SOURCE = "profiles/r2_ncu_full_cfg4.md"
 
 
-def ncu_traffic(kernel: str, cfg):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture of this workload
-    (profiles/r1b_traffic_<workload>.json.txt, written from profiles/r1b_sm100_ncu_full_cfg4.md), else None."""
-    path = os.path.join(ROOT, "profiles", f"r1b_traffic_{cfg.name}.json.txt")
-    if not os.path.exists(path):
-        return None
-    with open(path) as f:
-        table = json.load(f).get("dram_bytes_per_launch", {})
-    for k, v in table.items():
-        if k == kernel or k.startswith(kernel) or kernel.startswith(k):
-            return v
+def exp_floor_ms(name: str, cfg, sm_mhz: float) -> float | None:
+    """MUFU co-roofline: B*H*N^3 exps per pass at 148 SMs x 16 / clk."""
+    for key, passes in KERNEL_EXP_PASSES:
+        if key in name:
+            return passes * cfg.B * cfg.H * cfg.N ** 3 / (148 * 16 * sm_mhz * 1e6) * 1e3
     return None
 
 
@@ -233,6 +235,56 @@ def kernel_flop(name: str, cfg) -> float | None:
         if key in name:
             return units * base
     return None
+
+
+class DeviceProblem:
+    """One workload resident in HBM: inputs, outputs, workspace, and a step() = fwd + bwd through the C-ABI binding."""
+
+    def __init__(self, tri, cfg, rank, dev, keep_host=False):
+        import torch
+
+        x = tri_inputs.make_inputs(rank_config(cfg, rank))
+        tdt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
+        names = ("Q", "K", "V", "G", "bias", "dO")
+        host = {k: torch.from_numpy(x[k]).to(tdt) for k in names}
+        host["mask"] = None if x["mask"] is None else torch.from_numpy(x["mask"])
+        if keep_host:
+            host = {k: (None if v is None else v.pin_memory()) for k, v in host.items()}
+        self.host = host if keep_host else None
+        self.g = {k: (None if v is None else v.to(dev)) for k, v in host.items()}
+        B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
+        self.cfg, self.tri = cfg, tri
+        self.code = tri.BF16 if cfg.dtype == "bf16" else tri.F32
+        self.O = torch.empty_like(self.g["Q"])
+        self.LSE = torch.empty((B, N, H, N), dtype=torch.float32, device=dev)
+        self.grads = tuple(torch.empty_like(self.g["Q"]) for _ in range(4)) + (
+            torch.empty((B, H, N, N), dtype=torch.float32, device=dev),)
+        self.ws_bytes = max(tri.fwd_workspace_bytes(B, N, H, d, cfg.variant, self.code),
+                            tri.bwd_workspace_bytes(B, N, H, d, cfg.variant, self.code))
+        self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=dev)
+
+    def step(self):
+        g, cfg, tri = self.g, self.cfg, self.tri
+        tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], cfg.variant, O=self.O, LSE=self.LSE,
+                         workspace=self.ws)
+        tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], self.O, self.LSE, cfg.variant,
+                         out=self.grads, workspace=self.ws)
+
+
+def time_steps(prob, steps, warmup, barrier):
+    """W untimed steps, then K steps between two CUDA events on the launching stream (no other events inside)."""
+    import torch
+
+    for _ in range(warmup):
+        prob.step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        prob.step()
+    e1.record()
+    barrier()
+    return e0.elapsed_time(e1) / steps
 
 
 def run_ours(args, cfg):
@@ -260,70 +312,68 @@ def run_ours(args, cfg):
     tri.load()
     peaks = load_peaks()
 
-    # ---- inputs: seeded synthetic, rounded to bf16 once; each rank draws its own batch (weak scaling)
-    rcfg = rank_config(cfg, rank)
-    x = tri_inputs.make_inputs(rcfg)
-    tdt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
-    names = ("Q", "K", "V", "G", "bias", "dO")
-    host = {k: torch.from_numpy(x[k]).to(tdt).pin_memory() for k in names}
-    host["mask"] = None if x["mask"] is None else torch.from_numpy(x["mask"]).pin_memory()
-    del x
-    g = {k: (None if v is None else v.to(dev)) for k, v in host.items()}
-    B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
-    code = tri.BF16 if cfg.dtype == "bf16" else tri.F32
-    O = torch.empty_like(g["Q"])
-    LSE = torch.empty((B, N, H, N), dtype=torch.float32, device=dev)
-    grads = tuple(torch.empty_like(g["Q"]) for _ in range(4)) + (torch.empty((B, H, N, N), dtype=torch.float32, device=dev),)
-    ws_bytes = max(tri.fwd_workspace_bytes(B, N, H, d, cfg.variant, code), tri.bwd_workspace_bytes(B, N, H, d, cfg.variant, code))
-    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
-
-    def step():
-        tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], cfg.variant, O=O, LSE=LSE, workspace=ws)
-        tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], O, LSE, cfg.variant, out=grads,
-                         workspace=ws)
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- inputs: seeded synthetic, rounded to bf16 once; each rank draws its own batch (weak scaling)
+    prob = DeviceProblem(tri, cfg, rank, dev, keep_host=True)
+    B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
     for _ in range(args.warmup):
-        step()
+        prob.step()
     torch.cuda.synchronize()
     torch.cuda.reset_peak_memory_stats()
 
-    # ---- timed region: K steps, CUDA events on the launching stream, per-kernel events inside the library
+    # ---- timed region: K steps between two CUDA events, nothing else recorded inside
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     l0 = tri.launch_count()
-    tri.profile_begin()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
-    ms_total = e0.elapsed_time(e1)
-    prof = tri.profile_end()
+    ms_step = time_steps(prob, args.steps, 0, barrier)
     launches = tri.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     peak_bytes = torch.cuda.max_memory_allocated()
-    ms_total = max_over_ranks(ms_total, dev, world)
-    ms_step = ms_total / args.steps
+    ms_step = max_over_ranks(ms_step, dev, world)
     flop_all = model_flop(cfg) * world
     value = aggregate_value(cfg, world, ms_step)
 
+    # ---- per-kernel times: a second, separately profiled loop (events around every launch inside the library)
+    prof_steps = max(3, min(args.steps, 10))
+    tri.profile_begin()
+    for _ in range(prof_steps):
+        prob.step()
+    torch.cuda.synchronize()
+    prof = tri.profile_end()
+
+    # ---- the N=384 half of the metric (cfg3s / cfg3e), same protocol, rank 0's batch only
+    also = {}
+    if rank == 0 and cfg.name == "cfg4":
+        for name in ("cfg3s", "cfg3e"):
+            c3 = tri_inputs.CONFIGS[name]
+            p3 = DeviceProblem(tri, c3, 0, dev)
+            ms3 = time_steps(p3, max(20, args.steps), 5, torch.cuda.synchronize)
+            v3 = model_flop(c3) / (ms3 * 1e-3) / 1e12
+            also[name] = {"workload": workload_name(c3), "value": v3, "unit": UNIT, "ms_per_step": ms3,
+                          "pct_of_peak": {"spec_2250": 100 * v3 / SPEC_BF16_TFLOPS, "measured_burst": 100 * v3 / peaks["bf16_tflops"]},
+                          "l2": "inputs + outputs (10 x 75 MB) exceed the 126 MB L2; no flush"}
+            del p3
+        torch.cuda.empty_cache()
+
     # ---- e2e: the same step through tri_attn_step_host on pinned HOST buffers (H2D + D2H inside)
+    host = prob.host
+    ws_bytes = prob.ws_bytes
+    code = prob.code
     hout = {k: torch.empty_like(host["Q"]).pin_memory() for k in ("O", "dQ", "dK", "dV", "dG")}
     hout["LSE"] = torch.empty((B, N, H, N), dtype=torch.float32).pin_memory()
     hout["dBias"] = torch.empty((B, H, N, N), dtype=torch.float32).pin_memory()
-    del O, LSE, grads, ws, g
+    del prob
     torch.cuda.empty_cache()
     arena = torch.empty(tri.step_host_arena_bytes(B, N, H, d, cfg.variant, code), dtype=torch.uint8, device=dev)
     hin = dict(host)
     e2e_steps = max(2, min(args.steps, 5))
     tri.tri_attn_step_host(hin, hout, cfg.variant, arena)  # warm-up
     barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(e2e_steps):
         tri.tri_attn_step_host(hin, hout, cfg.variant, arena)
@@ -338,7 +388,7 @@ def run_ours(args, cfg):
     if rank != 0:
         return
 
-    # ---- roofline of the dominant kernel
+    # ---- roofline of the dominant kernel (times from the profiled loop)
     tot = sum(ms for _, ms in prof.values()) or 1.0
     kernels = {k: {"launches": n, "ms_per_launch": ms / n, "share": ms / tot} for k, (n, ms) in prof.items()}
     dom = max(prof, key=lambda k: prof[k][1])
@@ -346,6 +396,7 @@ def run_ours(args, cfg):
     dflop = kernel_flop(dom, cfg)
     sustained = args.steps * ms_step > 500.0  # a long step loop sits under the power cap
     peak = peaks["bf16_tflops_sustained" if sustained else "bf16_tflops"]
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
     if dflop is not None:
         ach = dflop / (dms / dn * 1e-3) / 1e12
         bound = "tensor" if "simt" not in dom else "alu"
@@ -353,14 +404,20 @@ def run_ours(args, cfg):
             # fp32 CUDA-core kernels: 148 SMs x 128 FMA lanes x 2 flop x max SM clock
             peak = 148 * 128 * 2 * 1.965e9 / 1e12
         roof = {"kernel": dom, "bound": bound, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": ncu_traffic(dom, cfg), "peak_source": peaks["source"] + (" sustained" if sustained else " burst") if bound == "tensor"
-                else "derived: 148 SM x 128 lanes x 2 x 1.965 GHz", "flop_per_launch": dflop, "ms_per_launch": dms / dn}
+                "traffic": None, "traffic_source": TRAFFIC_SOURCE,
+                "peak_source": peaks["source"] + (" sustained" if sustained else " burst") if bound == "tensor"
+                else "derived: 148 SM x 128 lanes x 2 x 1.965 GHz", "flop_per_launch": dflop, "flop_kind": "executed",
+                "ms_per_launch": dms / dn}
+        fl = exp_floor_ms(dom, cfg, sm_mhz)
+        if fl is not None:
+            roof["mufu_co_roofline"] = {"exp_floor_ms": fl, "frac": fl / (dms / dn),
+                                        "note": "one ex2 per logit and pass at 148 SM x 16/clk"}
     else:
         U = B * N * H * N * d * (2 if cfg.dtype == "bf16" else 4)
         bytes_ = 4 * U + B * N * H * N * 4  # preprocess: read dO,O,G, write dG + D
         ach = bytes_ / (dms / dn * 1e-3) / 1e9
         roof = {"kernel": dom, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]}
+                "frac": ach / peaks["hbm_gbs"], "traffic": None, "traffic_source": TRAFFIC_SOURCE, "peak_source": peaks["source"]}
 
     # ---- oracle on the host cores, bounded sample (~15 s)
     R = oracle_rows_for_budget(cfg, 15.0 / 1.0)
@@ -380,7 +437,8 @@ def run_ours(args, cfg):
                         "measured_sustained": 100 * value / world / peaks["bf16_tflops_sustained"], "peaks": peaks["source"]},
         "memory": {"peak_gb": peak_bytes / 1e9, "io_tensors_gb": (10 * U_bytes + 3 * B * H * N * N * 4) / 1e9,
                    "workspace_bytes": ws_bytes, "avoided_map_gb_bf16": B * H * N ** 3 * 2 / 1e9},
-        "kernels": kernels, "roofline": roof, "cpu_baseline": cpu,
+        "kernels": kernels, "kernels_source": f"separate profiled loop of {prof_steps} steps after the timed region",
+        "roofline": roof, "also": also, "cpu_baseline": cpu,
         "e2e": {"value": flop_all / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,

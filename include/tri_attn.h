@@ -36,17 +36,24 @@
  *     device: all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream).  Scratch space comes from `workspace` (device, 256-byte aligned, at
  *     least *_workspace_bytes() bytes, contents undefined on entry and exit).  workspace_bytes is
- *     O(B*H*N^2); nothing of size B*H*N^3 exists anywhere.
- *   - Outputs must not alias inputs or each other; outputs are overwritten (dBias is NOT
- *     accumulated into).  Results are bitwise reproducible run to run (no floating-point atomics).
+ *     O(B*H*N^2*d) (the backward keeps one dA = dO (.) sigmoid(G) tensor there); nothing of size
+ *     B*H*N^3 exists anywhere.
+ *   - Outputs (and the workspace) must not overlap inputs or each other: such a call returns
+ *     TRI_ERR_INVALID_ARG before any launch.  Outputs are overwritten (dBias is NOT accumulated into).  Results are bitwise reproducible run to run (no floating-point atomics).
  *   - tri_attn_step_host takes HOST pointers (pinned memory recommended) for every tensor plus a
- *     caller-owned DEVICE arena; it copies inputs in, runs forward + backward, copies results out,
- *     all on `cuda_stream`, and does not synchronise.
+ *     caller-owned DEVICE arena; it copies inputs in, runs forward + backward, copies results out
+ *     and does not synchronise.  Batch elements are independent problems, so it pipelines them:
+ *     host->device copies, compute and device->host copies of different elements overlap on two
+ *     library-owned copy streams forked from and joined back into `cuda_stream` with events (to the
+ *     caller it is still one unit of work on that stream).  Each element is solved as a B = 1
+ *     problem: identical to tri_attn_fwd/bwd on that element alone, which for dBias can differ in the
+ *     last bits from a B > 1 call (the row split of the deterministic reduction depends on B).
  *   - Errors: a tri_status is returned, nothing is thrown or aborted across the ABI.  Argument
  *     errors are detected before any launch.  Launch failures map to TRI_ERR_CUDA.
  *   - Supported: d in {16, 32, 64}, any N >= 1, dtype f32 or bf16.  bf16 with d == 32 and
- *     N % 128 == 0 runs on the tcgen05/TMA tensor-core kernels; every other combination runs on
- *     the fp32 CUDA-core kernels (fp32 needs them: the 1e-4 bound excludes TF32, reading A14).
+ *     N % 128 == 0 (N <= 2048) runs on the tcgen05/TMA tensor-core kernels; every other combination
+ *     runs on the fp32 CUDA-core kernels, ~30x slower (fp32 needs them: the 1e-4 bound excludes TF32,
+ *     reading A14); tri_attn_uses_tensor_cores() tells which.
  *     Anything else returns TRI_ERR_UNSUPPORTED.  There is no CPU path.
  */
 #ifndef TRI_ATTN_H_
@@ -105,6 +112,9 @@ TRI_API tri_status tri_attn_step_host(const void* hQ, const void* hK, const void
                               void* hdQ, void* hdK, void* hdV, void* hdG, float* hdBias,
                               int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
                               void* arena, size_t arena_bytes, void* cuda_stream);
+
+/* 1 if this problem runs on the tcgen05/TMA tensor-core kernels, 0 if on the fp32 CUDA-core kernels. */
+TRI_API int tri_attn_uses_tensor_cores(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);
 
 /* Number of kernel launches this library has enqueued since it was loaded (for bench accounting). */
 TRI_API unsigned long long tri_attn_launch_count(void);

@@ -28,6 +28,7 @@ SIGNATURES = {
     "tri_attn_bwd": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_step_host_arena_bytes": (_sz, [_i] * 6),
     "tri_attn_step_host": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
+    "tri_attn_uses_tensor_cores": (_i, [_i] * 6),
     "tri_attn_launch_count": (ctypes.c_ulonglong, []),
     "tri_attn_profile_begin": (None, []),
     "tri_attn_profile_end": (_i, [ctypes.c_char_p, _sz]),
@@ -98,6 +99,10 @@ def fwd_workspace_bytes(B, N, H, d, variant, dtype_code) -> int:
 
 def bwd_workspace_bytes(B, N, H, d, variant, dtype_code) -> int:
     return int(load().tri_attn_bwd_workspace_bytes(B, N, H, d, variant, dtype_code))
+
+
+def uses_tensor_cores(B, N, H, d, variant, dtype_code) -> bool:
+    return bool(load().tri_attn_uses_tensor_cores(B, N, H, d, variant, dtype_code))
 
 
 def launch_count() -> int:

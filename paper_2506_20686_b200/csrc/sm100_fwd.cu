@@ -430,7 +430,8 @@ extern "C" __attribute__((visibility("default"))) int tri_debug_mb(unsigned long
 }
 #endif
 
-bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0; }
+// N <= 2048: the fused dQ + dBias stage needs one cluster rank per two 64-key tiles (<= 16 ranks)
+bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0 && p.N <= 2048; }
 
 size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.N * (p.N / 64) * 8, 256); }
 

@@ -1,6 +1,8 @@
 // C-ABI entry points of libtri_attn.so (include/tri_attn.h): argument validation, workspace
 // accounting, kernel-family selection, and the host-buffer end-to-end step.
 #include <atomic>
+#include <mutex>
+#include <vector>
 #include <stdio.h>
 #include <string.h>
 
@@ -55,6 +57,19 @@ static bool size_ok(int B, int N, int H, int d) {
 }
 static bool al16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 
+// byte ranges of the tensors of a call; outputs must not overlap inputs or each other (include/tri_attn.h)
+struct Range { const void* p; size_t n; bool out; };
+static bool overlap(const Range& a, const Range& b) {
+    const uintptr_t a0 = (uintptr_t)a.p, b0 = (uintptr_t)b.p;
+    return a.p && b.p && a0 < b0 + b.n && b0 < a0 + a.n;
+}
+static bool aliasing(const Range* r, int n) {
+    for (int i = 0; i < n; ++i)
+        for (int j = i + 1; j < n; ++j)
+            if ((r[i].out || r[j].out) && overlap(r[i], r[j])) return true;
+    return false;
+}
+
 }  // namespace tri
 
 using namespace tri;
@@ -85,6 +100,13 @@ tri_status tri_attn_fwd(const void* Q, const void* K, const void* V, const void*
     if (!d_ok(d) || !size_ok(B, N, H, d)) return TRI_ERR_UNSUPPORTED;
     const size_t need = tri_attn_fwd_workspace_bytes(B, N, H, d, variant, dtype);
     if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TRI_ERR_WORKSPACE;
+    {
+        const size_t es = dtype == TRI_F32 ? 4 : 2, U = (size_t)B * N * H * N * d * es, P = (size_t)B * H * N * N;
+        const Range r[] = {{Q, U, false}, {K, U, false}, {V, U, false}, {G, U, false}, {bias, P * es, false},
+                           {mask, (size_t)B * N * N, false}, {O, U, true}, {LSE, (size_t)B * N * H * N * 4, true},
+                           {workspace, need, true}};
+        if (aliasing(r, 9)) return TRI_ERR_INVALID_ARG;
+    }
     Problem p = make_problem(B, N, H, d, variant);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (sm100_supported(p, dtype)) return sm100_fwd(p, Q, K, V, G, bias, mask, O, LSE, workspace, st);
@@ -104,6 +126,14 @@ tri_status tri_attn_bwd(const void* dO, const void* Q, const void* K, const void
     if (!d_ok(d) || !size_ok(B, N, H, d)) return TRI_ERR_UNSUPPORTED;
     const size_t need = tri_attn_bwd_workspace_bytes(B, N, H, d, variant, dtype);
     if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TRI_ERR_WORKSPACE;
+    {
+        const size_t es = dtype == TRI_F32 ? 4 : 2, U = (size_t)B * N * H * N * d * es, P = (size_t)B * H * N * N;
+        const Range r[] = {{dO, U, false}, {Q, U, false}, {K, U, false}, {V, U, false}, {G, U, false}, {bias, P * es, false},
+                           {mask, (size_t)B * N * N, false}, {O, U, false}, {LSE, (size_t)B * N * H * N * 4, false},
+                           {dQ, U, true}, {dK, U, true}, {dV, U, true}, {dG, U, true}, {dBias, P * 4, true},
+                           {workspace, need, true}};
+        if (aliasing(r, 15)) return TRI_ERR_INVALID_ARG;
+    }
     Problem p = make_problem(B, N, H, d, variant);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (sm100_supported(p, dtype))
@@ -146,6 +176,37 @@ size_t tri_attn_step_host_arena_bytes(int B, int N, int H, int d, tri_variant va
     return arena_layout(B, N, H, d, variant, dtype).total;
 }
 
+namespace {
+// copy streams and fork / join events of tri_attn_step_host (created once per process, never destroyed)
+struct HostPipe {
+    std::mutex mu;
+    cudaStream_t in = nullptr, out = nullptr;
+    std::vector<cudaEvent_t> ev;
+    bool ready = false;
+    bool init() {
+        if (ready) return true;
+        if (cudaStreamCreateWithFlags(&in, cudaStreamNonBlocking) != cudaSuccess) return false;
+        if (cudaStreamCreateWithFlags(&out, cudaStreamNonBlocking) != cudaSuccess) return false;
+        ready = true;
+        return true;
+    }
+    cudaEvent_t event(size_t i) {
+        while (ev.size() <= i) {
+            cudaEvent_t e = nullptr;
+            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+            ev.push_back(e);
+        }
+        return ev[i];
+    }
+};
+HostPipe g_pipes[64];  // one per device ordinal
+}  // namespace
+
+// Batch elements are independent problems (every tensor has B as its outermost axis), so the step runs as a
+// three-stage pipeline over b: H2D of element b+1 (copy stream) || forward + backward of element b (the caller's
+// stream) || D2H of element b-1 (second copy stream).  Inside an element the dO copy overlaps the forward and the
+// O / LSE read-back overlaps the backward.  Everything is forked from and joined back into `cuda_stream` with events,
+// so the call still behaves as one unit of work enqueued on that stream, and the host is never blocked.
 tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, const void* hG, const void* hbias,
                               const unsigned char* hmask, const void* hdO, void* hO, float* hLSE, void* hdQ,
                               void* hdK, void* hdV, void* hdG, float* hdBias, int B, int N, int H, int d,
@@ -158,35 +219,79 @@ tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, co
     const Arena a = arena_layout(B, N, H, d, variant, dtype);
     if (!arena || ((uintptr_t)arena & 255) || arena_bytes < a.total) return TRI_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    TRI_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return TRI_ERR_UNSUPPORTED;
+    HostPipe& g_pipe = g_pipes[dev];
+    std::lock_guard<std::mutex> lock(g_pipe.mu);
+    if (!g_pipe.init()) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: stream creation");
+    cudaStream_t sin = g_pipe.in, sout = g_pipe.out;
     char* base = (char*)arena;
     const size_t es = dtype == TRI_F32 ? 4 : 2;
-    const size_t Ub = (size_t)B * N * H * N * d * es;
-    const void* hin[5] = {hQ, hK, hV, hG, hdO};
-    for (int i = 0; i < 5; ++i) TRI_CUDA_CHECK(cudaMemcpyAsync(base + a.off[i], hin[i], Ub, cudaMemcpyHostToDevice, st));
-    TRI_CUDA_CHECK(cudaMemcpyAsync(base + a.off[10], hbias, (size_t)B * H * N * N * es, cudaMemcpyHostToDevice, st));
-    unsigned char* dmask = nullptr;
-    if (hmask) {
-        dmask = (unsigned char*)(base + a.off[11]);
-        TRI_CUDA_CHECK(cudaMemcpyAsync(dmask, hmask, (size_t)B * N * N, cudaMemcpyHostToDevice, st));
-    }
-    void *dQ_ = base + a.off[0], *dK_ = base + a.off[1], *dV_ = base + a.off[2], *dG_ = base + a.off[3];
-    void *ddO = base + a.off[4], *dO_ = base + a.off[5];
-    void *gQ = base + a.off[6], *gK = base + a.off[7], *gV = base + a.off[8], *gG = base + a.off[9];
-    void* dbias_in = base + a.off[10];
-    float* dLSE = (float*)(base + a.off[12]);
-    float* gBias = (float*)(base + a.off[13]);
-    void* ws = base + a.off[14];
-    tri_status s = tri_attn_fwd(dQ_, dK_, dV_, dG_, dbias_in, dmask, dO_, dLSE, B, N, H, d, variant, dtype, ws, a.ws, st);
-    if (s != TRI_OK) return s;
-    s = tri_attn_bwd(ddO, dQ_, dK_, dV_, dG_, dbias_in, dmask, dO_, dLSE, gQ, gK, gV, gG, gBias, B, N, H, d, variant,
-                     dtype, ws, a.ws, st);
-    if (s != TRI_OK) return s;
-    TRI_CUDA_CHECK(cudaMemcpyAsync(hO, dO_, Ub, cudaMemcpyDeviceToHost, st));
-    TRI_CUDA_CHECK(cudaMemcpyAsync(hLSE, dLSE, (size_t)B * N * H * N * 4, cudaMemcpyDeviceToHost, st));
+    // pipeline chunk = one batch element when its slices keep the 16-byte pointer alignment, else the whole batch
+    const bool split = B > 1 && ((size_t)H * N * N * es) % 16 == 0 && ((size_t)N * H * N * 4) % 16 == 0;
+    const int cb = split ? 1 : B, nchunk = B / cb;
+    // per-chunk sizes (bytes)
+    const size_t u = (size_t)cb * N * H * N * d * es, pb = (size_t)cb * H * N * N * es, mb = (size_t)cb * N * N,
+                 lb = (size_t)cb * N * H * N * 4, gb = (size_t)cb * H * N * N * 4;
+    // arena regions: 0-3 Q K V G | 4 dO | 5 O | 6-9 dQ dK dV dG | 10 bias | 11 mask | 12 LSE | 13 dBias | 14 workspace
+    auto U_ = [&](int r, int b) { return (void*)(base + a.off[r] + (size_t)b * u); };
+    size_t ne = 0;
+    cudaEvent_t e0 = g_pipe.event(ne++);
+    if (!e0) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: event creation");
+    // fork: the copy streams start after everything already enqueued on the caller's stream (the arena may be in use)
+    TRI_CUDA_CHECK(cudaEventRecord(e0, st));
+    TRI_CUDA_CHECK(cudaStreamWaitEvent(sin, e0, 0));
+    TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e0, 0));
+    const void* hin[4] = {hQ, hK, hV, hG};
     void* hout[4] = {hdQ, hdK, hdV, hdG};
-    void* dout[4] = {gQ, gK, gV, gG};
-    for (int i = 0; i < 4; ++i) TRI_CUDA_CHECK(cudaMemcpyAsync(hout[i], dout[i], Ub, cudaMemcpyDeviceToHost, st));
-    TRI_CUDA_CHECK(cudaMemcpyAsync(hdBias, gBias, (size_t)B * H * N * N * 4, cudaMemcpyDeviceToHost, st));
+    const size_t wf = tri_attn_fwd_workspace_bytes(cb, N, H, d, variant, dtype), wb = tri_attn_bwd_workspace_bytes(cb, N, H, d, variant, dtype);
+    void* ws = base + a.off[14];
+    for (int b = 0; b < nchunk; ++b) {
+        cudaEvent_t e_inA = g_pipe.event(ne++), e_inB = g_pipe.event(ne++), e_f = g_pipe.event(ne++), e_b = g_pipe.event(ne++);
+        if (!e_inA || !e_inB || !e_f || !e_b) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: event creation");
+        // ---- H2D of element b (copy stream): forward inputs, then dO
+        for (int i = 0; i < 4; ++i)
+            TRI_CUDA_CHECK(cudaMemcpyAsync(U_(i, b), (const char*)hin[i] + (size_t)b * u, u, cudaMemcpyHostToDevice, sin));
+        TRI_CUDA_CHECK(cudaMemcpyAsync(base + a.off[10] + (size_t)b * pb, (const char*)hbias + (size_t)b * pb, pb, cudaMemcpyHostToDevice, sin));
+        unsigned char* dmask = nullptr;
+        if (hmask) {
+            dmask = (unsigned char*)(base + a.off[11] + (size_t)b * mb);
+            TRI_CUDA_CHECK(cudaMemcpyAsync(dmask, hmask + (size_t)b * mb, mb, cudaMemcpyHostToDevice, sin));
+        }
+        TRI_CUDA_CHECK(cudaEventRecord(e_inA, sin));
+        TRI_CUDA_CHECK(cudaMemcpyAsync(U_(4, b), (const char*)hdO + (size_t)b * u, u, cudaMemcpyHostToDevice, sin));
+        TRI_CUDA_CHECK(cudaEventRecord(e_inB, sin));
+        // ---- compute of element b (caller's stream)
+        float* dLSE = (float*)(base + a.off[12] + (size_t)b * lb);
+        float* gBias = (float*)(base + a.off[13] + (size_t)b * gb);
+        void* dbias_in = base + a.off[10] + (size_t)b * pb;
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e_inA, 0));
+        tri_status s = tri_attn_fwd(U_(0, b), U_(1, b), U_(2, b), U_(3, b), dbias_in, dmask, U_(5, b), dLSE, cb, N, H, d, variant, dtype,
+                                    ws, wf, st);
+        if (s != TRI_OK) return s;
+        TRI_CUDA_CHECK(cudaEventRecord(e_f, st));
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e_inB, 0));
+        s = tri_attn_bwd(U_(4, b), U_(0, b), U_(1, b), U_(2, b), U_(3, b), dbias_in, dmask, U_(5, b), dLSE, U_(6, b), U_(7, b), U_(8, b),
+                         U_(9, b), gBias, cb, N, H, d, variant, dtype, ws, wb, st);
+        if (s != TRI_OK) return s;
+        TRI_CUDA_CHECK(cudaEventRecord(e_b, st));
+        // ---- D2H of element b (second copy stream): O, LSE while the backward runs, gradients after it
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e_f, 0));
+        TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hO + (size_t)b * u, U_(5, b), u, cudaMemcpyDeviceToHost, sout));
+        TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hLSE + (size_t)b * lb, dLSE, lb, cudaMemcpyDeviceToHost, sout));
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e_b, 0));
+        for (int i = 0; i < 4; ++i)
+            TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hout[i] + (size_t)b * u, U_(6 + i, b), u, cudaMemcpyDeviceToHost, sout));
+        TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hdBias + (size_t)b * gb, gBias, gb, cudaMemcpyDeviceToHost, sout));
+    }
+    // join: later work on the caller's stream waits for the last read-back (and for the copy-in stream, trivially done)
+    cudaEvent_t e1 = g_pipe.event(ne++), e2 = g_pipe.event(ne++);
+    if (!e1 || !e2) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: event creation");
+    TRI_CUDA_CHECK(cudaEventRecord(e1, sout));
+    TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e1, 0));
+    TRI_CUDA_CHECK(cudaEventRecord(e2, sin));
+    TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e2, 0));
     return TRI_OK;
 }
 
@@ -221,6 +326,11 @@ int tri_attn_profile_end(char* buf, size_t buflen) {
     }
     g_prof_n = 0;
     return na;
+}
+
+int tri_attn_uses_tensor_cores(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype) {
+    if (!shape_ok(B, N, H, d) || !enums_ok(variant, dtype) || !d_ok(d)) return 0;
+    return sm100_supported(make_problem(B, N, H, d, variant), dtype) ? 1 : 0;
 }
 
 unsigned long long tri_attn_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

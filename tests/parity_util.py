@@ -108,15 +108,18 @@ def outputs_to_starting(o: dict, variant: int) -> dict:
     return y
 
 
-def oracle_rows(oracle, xs: dict, rows):
+def oracle_rows(oracle, xs: dict, rows, with_dbias=False):
     """Oracle on a subset of broadcast rows r of a STARTING-form problem: exact O, LSE, dQ, dK, dV, dG of
-    those rows (rows are independent given the bias plane)."""
+    those rows (rows are independent given the bias plane); with_dbias adds those rows' partial sum of dBias."""
     rows = np.asarray(rows)
     sub = {k: xs[k][:, rows] for k in ("Q", "K", "V", "G", "dO")}
     m = None if xs["mask"] is None else xs["mask"][:, rows]
     O, LSE = oracle.fwd_start_general(sub["Q"], sub["K"], sub["V"], sub["G"], xs["bias"], m)
-    dQ, dK, dV, dG, _ = oracle.bwd_start_general(sub["dO"], sub["Q"], sub["K"], sub["V"], sub["G"], xs["bias"], m)
-    return dict(O=O, LSE=LSE, dQ=dQ, dK=dK, dV=dV, dG=dG)
+    dQ, dK, dV, dG, dBias = oracle.bwd_start_general(sub["dO"], sub["Q"], sub["K"], sub["V"], sub["G"], xs["bias"], m)
+    out = dict(O=O, LSE=LSE, dQ=dQ, dK=dK, dV=dV, dG=dG)
+    if with_dbias:
+        out["dBias"] = dBias
+    return out
 
 
 def oracle_dbias_queries(oracle, xs: dict, queries):

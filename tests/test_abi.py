@@ -60,6 +60,35 @@ def test_argument_validation_happens_before_any_launch(lib):
     assert b"UNSUPPORTED" in lib.tri_status_string(2)
 
 
+def test_overlapping_outputs_are_rejected_before_any_launch(lib):
+    """include/tri_attn.h: outputs (and the workspace) must not overlap inputs or each other -> TRI_ERR_INVALID_ARG."""
+    n0 = lib.tri_attn_launch_count()
+    B, N, H, d = 1, 32, 4, 32
+    U = B * N * H * N * d * 4
+    base = 1 << 30
+    a = [ctypes.c_void_p(base + i * (U + 4096)) for i in range(16)]  # fake, disjoint, aligned device addresses
+    ws = ctypes.c_void_p(base + 20 * (U + 4096))
+    wsb = 1 << 24
+    # O aliases Q
+    assert lib.tri_attn_fwd(a[0], a[1], a[2], a[3], a[4], None, a[0], a[6], B, N, H, d, 0, 0, ws, wsb, None) == 1
+    # LSE inside V
+    assert lib.tri_attn_fwd(a[0], a[1], a[2], a[3], a[4], None, a[5], ctypes.c_void_p(a[2].value + 64), B, N, H, d, 0, 0, ws, wsb, None) == 1
+    # workspace overlaps K
+    assert lib.tri_attn_fwd(a[0], a[1], a[2], a[3], a[4], None, a[5], a[6], B, N, H, d, 0, 0, a[1], wsb, None) == 1
+    # backward: dK aliases dQ; dG aliases dO
+    args = [a[0], a[1], a[2], a[3], a[4], a[5], None, a[6], a[7]]
+    assert lib.tri_attn_bwd(*args, a[8], a[8], a[10], a[11], a[12], B, N, H, d, 0, 0, ws, wsb, None) == 1
+    assert lib.tri_attn_bwd(*args, a[8], a[9], a[10], a[0], a[12], B, N, H, d, 0, 0, ws, wsb, None) == 1
+    assert lib.tri_attn_launch_count() == n0
+
+
+def test_tensor_core_path_query(lib):
+    assert lib.tri_attn_uses_tensor_cores(2, 768, 4, 32, 0, 1) == 1
+    assert lib.tri_attn_uses_tensor_cores(1, 200, 4, 32, 0, 1) == 0   # N not a multiple of 128: CUDA-core kernels
+    assert lib.tri_attn_uses_tensor_cores(1, 128, 4, 64, 0, 1) == 0   # d != 32
+    assert lib.tri_attn_uses_tensor_cores(1, 128, 4, 32, 0, 0) == 0   # fp32 (reading A14)
+
+
 @pytest.mark.parametrize("dtype", [0, 1])
 @pytest.mark.parametrize("variant", [0, 1])
 def test_workspace_is_quadratic_not_cubic(lib, variant, dtype):

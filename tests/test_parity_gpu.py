@@ -2,9 +2,9 @@
 the same seeded inputs, element by element, with the north_star error metric (A15):
 max|X_gpu - X_ref| / max|X_ref| <= 1e-4 (fp32) / 2e-2 (bf16 in, fp32 accumulate), per output tensor.
 
-Small cases compare every element; BASELINE.json's full-size configs (cfg3..cfg5) compare sampled
-broadcast rows (O, LSE, dQ, dK, dV, dG of whole rows: rows are independent given the bias plane) and
-sampled query lines of dBias summed over ALL rows (exact, see parity_util.oracle_dbias_queries).
+Every BASELINE.json config is compared element by element, all seven outputs: cfg1-cfg3 in one oracle call,
+cfg4 / cfg5 (N = 768 / 1024) in chunks of broadcast rows (rows are independent given the bias plane; dBias is the
+fp64 sum of the chunks' partial sums, ascending).  Only the N = 2048 case above the configs is sampled.
 """
 import numpy as np
 import pytest
@@ -132,27 +132,116 @@ def sampled_compare(oracle, cfg, n_rows=3, n_queries=3):
     return errs
 
 
+def chunked_full_compare(oracle, cfg, rows_per_chunk=32):
+    """Every element of all seven outputs at a full-size config: the oracle runs over chunks of broadcast rows."""
+    x = tri_inputs.make_inputs(cfg)
+    got, _ = pu.run_gpu(x, cfg.dtype, cfg.variant)
+    xs = pu.to_starting(x, cfg.variant)
+    gs = pu.outputs_to_starting(got, cfg.variant)
+    del x, got
+    names = ("O", "LSE", "dQ", "dK", "dV", "dG")
+    num = {k: 0.0 for k in names}
+    den = {k: 0.0 for k in names}
+    dB = np.zeros_like(gs["dBias"])
+    for r0 in range(0, cfg.N, rows_per_chunk):
+        rows = np.arange(r0, min(cfg.N, r0 + rows_per_chunk))
+        ref = pu.oracle_rows(oracle, xs, rows, with_dbias=True)
+        dB += ref.pop("dBias")
+        for k in names:
+            g, r = gs[k][:, rows], ref[k]
+            fin = np.isfinite(r)
+            assert np.array_equal(g[~fin], r[~fin]), (k, "non-finite entries differ")
+            assert np.isfinite(g[fin]).all(), k
+            if fin.any():
+                num[k] = max(num[k], float(np.max(np.abs(g[fin] - r[fin]))))
+                den[k] = max(den[k], float(np.max(np.abs(r[fin]))))
+    errs = {k: num[k] / den[k] for k in names}
+    errs["dBias"] = pu.rel_err(gs["dBias"], dB)
+    tol = pu.TOL[cfg.dtype]
+    print(cfg.name, "rel. errors (all elements):", {k: float(f"{v:.3g}") for k, v in errs.items()})
+    bad = {k: e for k, e in errs.items() if not e <= tol}
+    assert not bad, f"{cfg.name}: rel. error above {tol}: {bad} (all: {errs})"
+    return errs
+
+
 @pytest.mark.parametrize("name", ["cfg3s", "cfg3e"])
-def test_cfg3_n384_both_variants_sampled(tri, oracle, name):
-    sampled_compare(oracle, tri_inputs.CONFIGS[name])
+def test_cfg3_n384_both_variants_full(tri, oracle, name):
+    errs = full_compare(oracle, tri_inputs.CONFIGS[name])
+    print(name, "rel. errors (all elements):", {k: float(f"{v:.3g}") for k, v in errs.items()})
 
 
-def test_cfg4_n768_ragged_sampled(tri, oracle):
-    sampled_compare(oracle, tri_inputs.CONFIGS["cfg4"], n_rows=2, n_queries=2)
+def test_cfg4_n768_ragged_full(tri, oracle):
+    chunked_full_compare(oracle, tri_inputs.CONFIGS["cfg4"])
 
 
-def test_cfg5_n1024_ending_peaky_sampled_and_memory(tri, oracle):
-    """CFG5 + the memory claim: peak device memory stays far below the 8.6 GB bf16 map."""
+def test_cfg5_n1024_ending_peaky_full_and_memory(tri, oracle):
+    """CFG5, every element + the memory claim: peak device memory stays far below the 8.6 GB bf16 map."""
     import torch
 
     torch.cuda.empty_cache()
     torch.cuda.reset_peak_memory_stats()
     base = torch.cuda.memory_allocated()
-    sampled_compare(oracle, tri_inputs.CONFIGS["cfg5"], n_rows=2, n_queries=2)
+    chunked_full_compare(oracle, tri_inputs.CONFIGS["cfg5"])
     peak = torch.cuda.max_memory_allocated() - base
     U = 1024 * 4 * 1024 * 32 * 2
     assert peak < 14 * U, f"peak {peak / 1e9:.2f} GB: something of O(N^3) was allocated?"
     assert peak < 4 * 1024 ** 3 * 2 * 0.6
+
+
+@pytest.mark.parametrize("variant", [STARTING, ENDING])
+def test_dead_key_tiles_on_the_tensor_core_path(tri, oracle, variant):
+    """N=384 (three 128-key blocks, six 64-key tiles) with a general [B,N,N] mask whose dead tiles differ per broadcast
+    row: leading block masked with later ones live (running max still -inf after the first tiles), two
+    leading blocks masked, only the last 64-key tile visible, a middle block masked, one dead 64-key tile (ragged) that
+    moves with the row, fully masked rows, and unmasked rows.  Every element of every output against the oracle."""
+    N = 384
+    cfg = tri_inputs.small_config(1, N, 2, 32, "bf16", variant, 1.5, "none", seed=611)
+    x = tri_inputs.make_inputs(cfg)
+    m = np.ones((1, N, N), np.uint8)  # starting form: m[b, row, key]
+    for r in range(N):
+        kind = r % 6
+        if kind == 1:
+            m[0, r, :128] = 0
+        elif kind == 2:
+            m[0, r, :256] = 0
+        elif kind == 3:
+            m[0, r, :N - 64] = 0
+        elif kind == 4:
+            m[0, r, 128:256] = 0
+        elif kind == 5:
+            m[0, r, 64 * (r % 5):64 * (r % 5) + 64 + (r % 3)] = 0
+    m[0, 7, :] = 0
+    m[0, N - 2, :] = 0
+    x["mask"] = m if variant == STARTING else np.ascontiguousarray(np.swapaxes(m, -1, -2))
+    got, _ = pu.run_gpu(x, "bf16", variant)
+    ref = pu.run_oracle(oracle, x, variant)
+    errs = pu.assert_close(got, ref, pu.TOL["bf16"], what=f"dead-tiles-v{variant}")
+    print("dead tiles, variant", variant, {k: float(f"{v:.3g}") for k, v in errs.items()})
+    assert np.isneginf(got["LSE"]).sum() == np.isneginf(ref["LSE"]).sum() == 2 * 2 * N
+
+
+@pytest.mark.parametrize("variant", [STARTING, ENDING])
+def test_single_visible_key_rows(tri, oracle, variant):
+    """Rows that see only their LAST key (five dead tiles, then one live column): P is a delta, so O = sigmoid(G) V_k,
+    LSE = the one score, and dS = P (dP - D) is exactly zero.  The flash backward takes D = rowsum(dO . O) from the
+    bf16-rounded O (reading A3) and dP from the bf16-rounded dA, so it returns a pure cancellation residue
+    there instead of 0: ~2^-9 sqrt(d) |dO||V| per logit, i.e. a few percent of max|dK| once summed over the queries.
+    That residue is inherent in the method with bf16 storage, not a kernel defect: O, LSE, dV, dG, dBias must meet the
+    2e-2 bound; dQ / dK are held to 1e-1 and must be far below the size of the ordinary rows' gradients."""
+    N = 384
+    cfg = tri_inputs.small_config(1, N, 2, 32, "bf16", variant, 1.5, "none", seed=612)
+    x = tri_inputs.make_inputs(cfg)
+    m = np.ones((1, N, N), np.uint8)  # starting form: m[b, row, key]
+    m[0, ::3, :N - 1] = 0
+    x["mask"] = m if variant == STARTING else np.ascontiguousarray(np.swapaxes(m, -1, -2))
+    got, _ = pu.run_gpu(x, "bf16", variant)
+    ref = pu.run_oracle(oracle, x, variant)
+    errs = {k: pu.rel_err(got[k], ref[k]) for k in pu.OUT_NAMES}
+    print("single visible key, variant", variant, {k: float(f"{v:.3g}") for k, v in errs.items()})
+    for k in ("O", "LSE", "dV", "dG", "dBias"):
+        assert errs[k] <= pu.TOL["bf16"], (k, errs)
+    for k in ("dQ", "dK"):
+        assert errs[k] <= 1e-1, (k, errs)
 
 
 def test_tile_boundary_metamorphic(tri):
@@ -195,6 +284,32 @@ def test_step_host_end_to_end_matches_device_path(tri):
         assert torch.equal(hout[k].view(torch.uint8), dev[k].cpu().view(torch.uint8)), k
 
 
+def test_step_host_pipelines_batch_elements(tri, oracle):
+    """B = 3: tri_attn_step_host overlaps the copies and the compute of different batch elements; each element must be
+    bitwise what tri_attn_fwd / tri_attn_bwd give for that element alone, and the whole must match the oracle."""
+    import torch
+
+    cfg = tri_inputs.small_config(3, 256, 2, 32, "bf16", ENDING, 1.0, "lengths:200,256,131", seed=97)
+    x = tri_inputs.make_inputs(cfg)
+    hin = {k: pu.to_torch(x[k], cfg.dtype, "cpu").pin_memory() for k in ("Q", "K", "V", "G", "bias", "dO")}
+    hin["mask"] = torch.from_numpy(x["mask"]).pin_memory()
+    B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
+    hout = {k: torch.empty_like(hin["Q"]).pin_memory() for k in ("O", "dQ", "dK", "dV", "dG")}
+    hout["LSE"] = torch.empty((B, N, H, N), dtype=torch.float32).pin_memory()
+    hout["dBias"] = torch.empty((B, H, N, N), dtype=torch.float32).pin_memory()
+    arena = torch.empty(tri.step_host_arena_bytes(B, N, H, d, cfg.variant, tri.BF16), dtype=torch.uint8, device="cuda")
+    for _ in range(2):  # twice: the second call reuses the arena while the first one's copies may still be in flight
+        tri.tri_attn_step_host(hin, hout, cfg.variant, arena)
+    torch.cuda.synchronize()
+    for b in range(B):
+        xb = {k: (None if v is None else v[b:b + 1]) for k, v in x.items()}
+        _, dev = pu.run_gpu(xb, cfg.dtype, cfg.variant)
+        for k in pu.OUT_NAMES:
+            assert torch.equal(hout[k][b:b + 1].contiguous().view(torch.uint8), dev[k].cpu().view(torch.uint8)), (k, b)
+    got = {k: hout[k].float().numpy().astype(np.float64) for k in pu.OUT_NAMES}
+    pu.assert_close(got, pu.run_oracle(oracle, x, cfg.variant), pu.TOL["bf16"], what="step_host B=3")
+
+
 def test_bitwise_determinism_with_row_split_dbias(tri):
     """N=384: the dBias kernel splits the broadcast-row axis over 4 CTAs per tile and a second pass adds the
     partial planes in a fixed order -- the result must still be bitwise reproducible (A16)."""
@@ -206,34 +321,6 @@ def test_bitwise_determinism_with_row_split_dbias(tri):
     _, b = pu.run_gpu(x, cfg.dtype, cfg.variant)
     for k in pu.OUT_NAMES:
         assert torch.equal(a[k].view(torch.uint8), b[k].view(torch.uint8)), k
-
-
-_ALT_SCRIPT = r"""
-import sys, os
-sys.path.insert(0, os.getcwd()); sys.path.insert(0, os.path.join(os.getcwd(), "tests"))
-import oracle, parity_util as pu, tri_inputs
-oracle.build()
-for variant in (0, 1):
-    cfg = tri_inputs.small_config(1, 256, 2, 32, "bf16", variant, 2.0, "tail:9", seed=77)
-    x = tri_inputs.make_inputs(cfg)
-    got, _ = pu.run_gpu(x, "bf16", variant)
-    ref = pu.run_oracle(oracle, x, variant)
-    pu.assert_close(got, ref, pu.TOL["bf16"], what="alt-kernels v%d" % variant)
-print("ALT OK")
-"""
-
-
-def test_alternate_kernels_parity(tri):
-    """The warp-specialised forward (TRI_FWD_WS=1) and the software-pipelined dQ (TRI_DQ_WS=1) are kept for A/B:
-    they must stay parity-green too.  The switches are read once per process, hence the subprocess."""
-    import os
-    import subprocess
-    import sys
-
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    env = dict(os.environ, TRI_FWD_WS="1", TRI_DQ_WS="1")
-    r = subprocess.run([sys.executable, "-c", _ALT_SCRIPT], cwd=root, env=env, capture_output=True, text=True, timeout=600)
-    assert r.returncode == 0 and "ALT OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
 
 
 def test_n2048_beyond_the_configs_sampled(tri, oracle):
