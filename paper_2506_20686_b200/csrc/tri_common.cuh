@@ -91,6 +91,11 @@ tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int 
 // keep flags -> one 64-bit word per (b, row, 64-key tile), rows / keys in the variant's sense
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st);
 size_t sm100_maskbits_bytes(const Problem& p);
+// dK / dV stage (sm100_dkdv.cu): NL / ND are fp32 [B,N,H,N] scratch arrays of sm100_dkdv2_aux_bytes() each
+size_t sm100_dkdv2_aux_bytes(const Problem& p);
+tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, const void* K, const void* V, const void* bias_kq,
+                              const unsigned long long* maskbits, const float* LSE, const float* Dws, float* NL, float* ND,
+                              void* dK, void* dV, cudaStream_t st);
 // fused dQ + dBias stage (sm100_dqdb.cu): cluster size (0 = shape not covered), row split, persistent grid, launch
 int sm100_dqdb_cluster(int N);
 constexpr int kDqdbMaxSplit = 8;  // the workspace holds this many partial dBias planes
