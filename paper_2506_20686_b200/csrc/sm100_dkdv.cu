@@ -53,13 +53,15 @@ struct DkdvSmem {
 };
 
 struct ItemK { int b, h, k0, r0; };
+// key block fastest: the CTAs that run concurrently share the Q / dA rows of a few row triples (read once from HBM,
+// then from L2) instead of streaming the whole pair tensor once per key block
 __device__ __forceinline__ ItemK decode_itemk(int item, int N, int H, int NT3) {
     ItemK it;
     const int NKB = N / BKEY;
-    it.r0 = (item % NT3) * NGK;
-    int t = item / NT3;
-    it.k0 = (t % NKB) * BKEY;
-    const int bh = t / NKB;
+    it.k0 = (item % NKB) * BKEY;
+    int t = item / NKB;
+    it.r0 = (t % NT3) * NGK;
+    const int bh = t / NT3;
     it.b = bh / H;
     it.h = bh % H;
     return it;
