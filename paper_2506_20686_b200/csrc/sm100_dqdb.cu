@@ -123,13 +123,14 @@ __device__ __forceinline__ void dqdb_chunk(const uint32_t (&sr)[16], const uint3
 }
 
 struct Item2 { int b, h, q0, rb; };
+// query block fastest: clusters that run concurrently work on the same rows (K_r, V_r shared through L2)
 __device__ __forceinline__ Item2 decode_item2(int item, int N, int H, int G, int NR) {
     Item2 it;
     const int NQB = N / BQ;
-    it.rb = (item % G) * NR;
-    int t = item / G;
-    it.q0 = (t % NQB) * BQ;
-    const int bh = t / NQB;
+    it.q0 = (item % NQB) * BQ;
+    int t = item / NQB;
+    it.rb = (t % G) * NR;
+    const int bh = t / G;
     it.b = bh / H;
     it.h = bh % H;
     return it;

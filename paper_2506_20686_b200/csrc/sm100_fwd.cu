@@ -51,10 +51,9 @@ struct FwdSmem {
     static constexpr int total = bar_off + n_bars * 8 + 16 + 1024;     // + tmem slot + alignment slack
 };
 
-#ifdef TRI_DEBUG_MB
-__device__ unsigned long long g_dbg_mb[1 << 16];
-#endif
 struct Item { int b, h, q0, r4; };
+// row quad fastest (measured: query block fastest halves the K / V re-reads from HBM but is 4 % slower at cfg5, where
+// the ending-node rows are 64-byte neighbours in memory and concurrent quads share DRAM pages)
 __device__ __forceinline__ Item decode_item(int item, int N, int H) {
     const int NRQ = N / NG, NQB = N / BQ;
     Item it;
@@ -112,9 +111,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
 
     if (warp >= NG * 4) {
         // =============================== helper warpgroup ===============================
-#ifndef TRI_NO_SETMAXNREG
         setmaxnreg_dec<40>();
-#endif
         if (warp == NG * 4) {
             // ---- TMA producer: bias tile of (item, kt) once, then (Q at kt = 0,) K, V of every group ----
             int kst = 0, kph = 0, bst = 0, bph = 0;
@@ -211,9 +208,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         }
     } else {
         // =============================== softmax groups ===============================
-#ifndef TRI_NO_SETMAXNREG
         setmaxnreg_inc<104>();  // 512 x 104 + 128 x 40 <= 640 x 96 (the launch allocation)
-#endif
         const int g = warp >> 2;
         const int row = tid & 127;                                  // query row inside the block = TMEM lane
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
@@ -233,10 +228,6 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
             for (int kt = 0; kt < TPR; ++kt, ++n) {
                 const uint64_t mb = mb_next;
                 if (mrow && kt + 1 < TPR) mb_next = ldg_u64(mrow + kt + 1);
-#ifdef TRI_DEBUG_MB
-                if ((tid & 31) == 0)
-                    g_dbg_mb[(((((it.b * p.H + it.h) * (N / BQ) + it.q0 / BQ) * N + r) * NW + kt) * 4 + (warp & 3)) & 0xffff] = mb;
-#endif
                 mbar_wait(s_full + g, n & 1);
                 tc_fence_after();
                 uint32_t raw[BK];
@@ -424,11 +415,6 @@ tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bi
 }
 
 int sm100_sm_count() { return sm_count(); }
-#ifdef TRI_DEBUG_MB
-extern "C" __attribute__((visibility("default"))) int tri_debug_mb(unsigned long long* host, int n) {
-    return (int)cudaMemcpyFromSymbol(host, g_dbg_mb, (size_t)n * 8);
-}
-#endif
 
 // N <= 2048: the fused dQ + dBias stage needs one cluster rank per two 64-key tiles (<= 16 ranks)
 bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0 && p.N <= 2048; }
