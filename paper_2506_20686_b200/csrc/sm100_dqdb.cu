@@ -16,13 +16,14 @@
 //                32-key halves of the tile per row (S / dP ping-pong in TMEM, so the MMAs of one half run under the math
 //                of the other): p = exp2(S*scale*log2e + log2e*bias - LSE*log2e), dS = p (dP - D), dBias += dS,
 //                dS -> bf16 -> TMEM;
-//   warp 8       TMA producer: per row Q_r, dA_r (128 x 32) and K_r, V_r (128 x 32) into a 3-stage ring; per work item
-//                the bias tiles of the groups;
-//   warp 9       S / dP issuer: per row, Q_r and dA_r go shared memory -> TMEM once (tcgen05.cp), so the eight
-//                S = Q K^T, dP = dA V^T MMAs of the row (per group and half, TS form) only read their 32-key B operands
-//                from shared memory;
-//   warp 10      dQ issuer: dQ += dS K (TS, M128 N32 K2x16) in a fixed (half, group) order into a double-buffered
-//                accumulator;
+//   warp 8       feeder: TMA of Q_r, dA_r (128 x 32) and K_r, V_r (128 x 32) into a 3-stage ring, the bias tiles of the
+//                groups per work item, and the shared memory -> TMEM copy (tcgen05.cp) of Q_r, dA_r one row ahead;
+//   warps 9-10   one S / dP issuer per group: S = Q K^T, dP = dA V^T per half (TS form: A = Q_r / dA_r in TMEM, so shared
+//                memory only serves the 32-key B operands);
+//   warp 11      dQ issuer: dQ += dS K (TS, M128 N32 K2x16) in a fixed (half, group) order into one of four accumulators.
+//                (Measured on this B200: one thread issues a tcgen05.mma every ~50 clk, a tcgen05.cp every ~107 clk and a
+//                tcgen05.commit every ~142 clk, and different warps issue concurrently -- so the tensor work of a row is
+//                spread over four warps and commits are kept to one per hand-off.)
 //   warps 12-15  dQ reducer: partial dQ of a row: TMEM -> registers -> + inbox -> next rank's inbox (st.async into
 //                distributed shared memory, completion counted on the receiver's mbarrier) or, on the last rank, global.
 #include <cuda_runtime.h>
@@ -63,8 +64,9 @@ struct DqdbSmem {
     static constexpr int b_s_full = b_bias_free + 1;      // [NGB][2] S, dP of the half in TMEM
     static constexpr int b_consumed = b_s_full + 2 * NGB; // [NGB][2] S, dP of the half are in registers
     static constexpr int b_ds_ready = b_consumed + 2 * NGB;  // [NGB][2] dS of the half in TMEM
-    static constexpr int b_ds_free = b_ds_ready + 2 * NGB;   // [NGB][2] dQ MMAs of the half have read dS
-    static constexpr int b_dq_full = b_ds_free + 2 * NGB; // [NDQ] partial dQ of the row complete
+    static constexpr int b_qa_ready = b_ds_ready + 2 * NGB;  // [2] Q_r, dA_r of a row copied into TMEM
+    static constexpr int b_qa_free = b_qa_ready + 2;         // [2] every S / dP MMA that reads the buffer has completed
+    static constexpr int b_dq_full = b_qa_free + 2;       // [NDQ] partial dQ of the row complete (= its dS halves are free)
     static constexpr int b_dq_free = b_dq_full + NDQ;     // [NDQ] reducer has it in registers
     static constexpr int b_in_full = b_dq_free + NDQ;       // [NIN] lower rank's st.async bytes landed in my inbox slot
     static constexpr int b_out_free = b_in_full + NIN;    // [NIN] upper rank read its inbox slot (remote arrivals)
@@ -158,7 +160,8 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     uint64_t* s_full = bars + L::b_s_full;
     uint64_t* consumed = bars + L::b_consumed;
     uint64_t* ds_ready = bars + L::b_ds_ready;
-    uint64_t* ds_free = bars + L::b_ds_free;
+    uint64_t* qa_ready = bars + L::b_qa_ready;
+    uint64_t* qa_free = bars + L::b_qa_free;
     uint64_t* dq_full = bars + L::b_dq_full;
     uint64_t* dq_free = bars + L::b_dq_free;
     uint64_t* in_full = bars + L::b_in_full;
@@ -184,8 +187,9 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         mbar_init(bias_full, 1);
         mbar_init(bias_free, nt * 4);
         for (int i = 0; i < 2 * NGB; ++i) {
-            mbar_init(s_full + i, 1); mbar_init(consumed + i, 4); mbar_init(ds_ready + i, 4); mbar_init(ds_free + i, 1);
+            mbar_init(s_full + i, 1); mbar_init(consumed + i, 4); mbar_init(ds_ready + i, 4);
         }
+        for (int i = 0; i < 2; ++i) { mbar_init(qa_ready + i, 1); mbar_init(qa_free + i, nt * 4); }
         for (int i = 0; i < NDQ; ++i) { mbar_init(dq_full + i, 1); mbar_init(dq_free + i, 4); }
         for (int i = 0; i < NIN; ++i) { mbar_init(in_full + i, 1); mbar_init(out_free + i, 4); }
         fence_barrier_init();
@@ -200,8 +204,26 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     if (warp >= NGB * 4 && warp < NGB * 4 + 4) {
         // =============================== helper warpgroup ===============================
         setmaxnreg_dec<40>();
+        const uint32_t opbase = smem_u32(sOp);
         if (warp == NGB * 4) {
-            // ---- TMA producer ----
+            // ---- feeder: TMA loads NST - 1 rows ahead, tcgen05.cp of Q_r / dA_r one row ahead ----
+            auto stage_qa = [&](int m) {  // Q_r, dA_r of row m (this CTA's m-th row): ring stage -> TMEM buffer m & 1
+                const int s = m % NST;
+                mbar_wait(full + s, (m / NST) & 1);
+                if (m >= 2) mbar_wait(qa_free + (m & 1), ((m >> 1) - 1) & 1);  // the S / dP MMAs of row m - 2 are done with it
+                tc_fence_after();
+                const uint32_t st = opbase + s * STAGE_BYTES;
+                const uint64_t dq = make_desc_sw64(st), da = make_desc_sw64(st + QT_BYTES);
+                const uint32_t tQ = tmem + TM_QA + (m & 1) * 32;
+                if (elect_one()) {
+                    tmem_cp_128x256b(tQ, dq);
+                    tmem_cp_128x256b(tQ + 8, dq + 2);
+                    tmem_cp_128x256b(tQ + 16, da);
+                    tmem_cp_128x256b(tQ + 24, da + 2);
+                    mma_commit(qa_ready + (m & 1));
+                }
+                __syncwarp();
+            };
             int n = 0;
             for (int il = 0; il < n_my; ++il) {
                 const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
@@ -227,65 +249,41 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                         tma_load_5d(st + 2 * QT_BYTES + NGB * KT_BYTES, &tmV, full + s, 0, k0, it.rb + r, it.h, it.b);
                     }
                     __syncwarp();
+                    // the row loaded NST - 2 iterations ago goes to TMEM (its TMA has landed; it is one row ahead of the MMAs)
+                    if (n >= NST - 2) stage_qa(n - (NST - 2));
                 }
             }
-        } else if (warp == NGB * 4 + 1) {
-            // ---- S / dP issuer (warp-uniform control flow; one elected lane issues and commits) ----
-            // Q_r, dA_r of a row go shared memory -> TMEM once (tcgen05.cp, two rows ahead); a half gets its next S, dP as
-            // soon as the compute group has the previous row's values of that half in registers.  tcgen05.cp / .mma of
-            // one thread execute in issue order, so the copies need no barrier of their own.
+            for (int m = (NRtot > NST - 2 ? NRtot - (NST - 2) : 0); m < NRtot; ++m) stage_qa(m);
+        } else if (warp <= NGB * 4 + NGB) {
+            // ---- S / dP issuer of group g (warp-uniform control flow; one elected lane issues and commits) ----
+            const int g = warp - (NGB * 4 + 1);
             constexpr uint32_t idesc = make_idesc(128, BH, false, false);  // B = K / V rows, K-major
-            const uint32_t opbase = smem_u32(sOp);
-            auto stage_qa = [&](int m, int s) {
-                mbar_wait(full + s, (m / NST) & 1);
-                tc_fence_after();
-                const uint32_t st = opbase + s * STAGE_BYTES;
-                const uint64_t dq = make_desc_sw64(st), da = make_desc_sw64(st + QT_BYTES);
-                const uint32_t tQ = tmem + TM_QA + (m & 1) * 32;
-                if (elect_one()) {
-                    tmem_cp_128x256b(tQ, dq);
-                    tmem_cp_128x256b(tQ + 8, dq + 2);
-                    tmem_cp_128x256b(tQ + 16, da);
-                    tmem_cp_128x256b(tQ + 24, da + 2);
-                }
-                __syncwarp();
-            };
-            auto issue_sdp = [&](int n, int s, int g, int h) {
-                const uint32_t st = opbase + s * STAGE_BYTES + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2);
-                const uint64_t dk = make_desc_sw64(st), dv = make_desc_sw64(st + NGB * KT_BYTES);
-                const uint32_t tS = tmem + g * TM_GROUP + h * TM_HALF, tDP = tS + 32;
-                const uint32_t tQ = tmem + TM_QA + (n & 1) * 32, tA = tQ + 16;
-                if (elect_one()) {
-                    mma_ts(tS, tQ, dk, idesc, 0);
-                    mma_ts(tS, tQ + 8, dk + 2, idesc, 1);
-                    mma_ts(tDP, tA, dv, idesc, 0);
-                    mma_ts(tDP, tA + 8, dv + 2, idesc, 1);
-                    mma_commit(s_full + g * 2 + h);
-                }
-                __syncwarp();
-            };
-            if (NRtot > 0) stage_qa(0, 0);
-            int s = 0, s1 = 1 % NST;  // ring stages of row n and row n + 1
-            for (int n = 0; n < NRtot; ++n) {
-                for (int h = 0; h < 2; ++h) {
-                    for (int g = 0; g < nt; ++g) {
-                        if (n > 0) {
-                            mbar_wait(consumed + g * 2 + h, (n - 1) & 1);
-                            tc_fence_after();
+            if (g < nt) {
+                int s = 0;
+                for (int n = 0; n < NRtot; ++n) {
+                    mbar_wait(qa_ready + (n & 1), (n >> 1) & 1);  // Q_r, dA_r in TMEM (this also means the row's TMA has landed)
+                    for (int h = 0; h < 2; ++h) {
+                        if (n > 0) mbar_wait(consumed + g * 2 + h, (n - 1) & 1);
+                        tc_fence_after();
+                        const uint32_t st = opbase + s * STAGE_BYTES + 2 * QT_BYTES + g * KT_BYTES + h * (BH * DH * 2);
+                        const uint64_t dk = make_desc_sw64(st), dv = make_desc_sw64(st + NGB * KT_BYTES);
+                        const uint32_t tS = tmem + g * TM_GROUP + h * TM_HALF, tDP = tS + 32;
+                        const uint32_t tQ = tmem + TM_QA + (n & 1) * 32, tA = tQ + 16;
+                        if (elect_one()) {
+                            mma_ts(tS, tQ, dk, idesc, 0);
+                            mma_ts(tS, tQ + 8, dk + 2, idesc, 1);
+                            mma_ts(tDP, tA, dv, idesc, 0);
+                            mma_ts(tDP, tA + 8, dv + 2, idesc, 1);
+                            mma_commit(s_full + g * 2 + h);
                         }
-                        issue_sdp(n, s, g, h);
+                        __syncwarp();
                     }
-                    // next row's Q / dA -> the other TMEM buffer (every S / dP MMA of row n - 1, its last reader, is issued;
-                    // the row landed in shared memory long ago, so this wait does not block the second halves)
-                    if (h == 0 && n + 1 < NRtot) stage_qa(n + 1, s1);
+                    if (++s == NST) s = 0;
                 }
-                if (++s == NST) s = 0;
-                if (++s1 == NST) s1 = 0;
             }
-        } else if (warp == NGB * 4 + 2) {
+        } else {
             // ---- dQ issuer: dQ_r += dS(g, h) K_r[keys 32h .. 32h+31 of tile g], strictly in (row, half, group) order ----
             constexpr uint32_t idescO = make_idesc(128, DH, false, true);  // B = K rows as [key][d], MN-major
-            const uint32_t opbase = smem_u32(sOp);
             int s = 0;
             for (int n = 0; n < NRtot; ++n) {
                 const int j = n % NDQ;
@@ -301,10 +299,12 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                         if (elect_one()) {
                             mma_ts(tDQ, tDS, dk, idescO, first ? 0u : 1u);
                             mma_ts(tDQ, tDS + 8, dk + 64, idescO, 1u);
-                            mma_commit(ds_free + g * 2 + h);
                             if (last) {
+                                // one commit per hand-off: the row's partial dQ is complete -- which also tells the compute
+                                // groups that every dS half of the row has been read -- and the ring stage is free (the
+                                // S / dP MMAs and copies of the row completed before its dS existed)
                                 mma_commit(dq_full + j);
-                                mma_commit(freeb + s);  // S / dP MMAs and copies of the row completed before its dS existed
+                                mma_commit(freeb + s);
                             }
                         }
                         __syncwarp();
@@ -363,6 +363,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                         const uint32_t mh = (uint32_t)(mb >> (h * 32));
                         mbar_wait(s_full + g * 2 + h, n & 1);
                         tc_fence_after();
+                        if (h == 1) warp_arrive(qa_free + (n & 1));  // my group's S / dP MMAs of the row are complete
                         uint32_t dsb[2][8];
 #pragma unroll
                         for (int ch = 0; ch < 2; ++ch) {  // 16 key columns at a time
@@ -380,7 +381,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                                        mh != 0xffffffffu);
                         }
                         if (n > 0) {  // the dQ MMAs of the previous row have read this half's dS columns
-                            mbar_wait(ds_free + g * 2 + h, (n - 1) & 1);
+                            mbar_wait(dq_full + (n - 1) % NDQ, ((n - 1) / NDQ) & 1);
                             tc_fence_after();
                         }
                         tmem_st8(tDS, dsb[0]);
