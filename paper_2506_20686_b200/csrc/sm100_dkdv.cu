@@ -48,7 +48,8 @@ struct DkdvSmem {
     static constexpr int b_p_ready = b_s_full + NGK;                  // [NGK] P^T, dS^T of the unit in TMEM
     static constexpr int b_acc_full = b_p_ready + NGK;                // [NGK] dV, dK of the row complete
     static constexpr int b_acc_free = b_acc_full + NGK;               // [NGK] the group has them in registers
-    static constexpr int n_bars = b_acc_free + NGK;
+    static constexpr int b_tok = b_acc_free + NGK;                    // [NGK][4] math-phase token of (group, scheduler quarter)
+    static constexpr int n_bars = b_tok + NGK * 4;
     static constexpr int total = bar_off + n_bars * 8 + 16 + 1024;
 };
 
@@ -116,6 +117,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     uint64_t* p_ready = bars + L::b_p_ready;
     uint64_t* acc_full = bars + L::b_acc_full;
     uint64_t* acc_free = bars + L::b_acc_free;
+    uint64_t* tok = bars + L::b_tok;
     uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -132,6 +134,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         for (int i = 0; i < NGK; ++i) {
             mbar_init(s_full + i, 1); mbar_init(p_ready + i, 4); mbar_init(acc_full + i, 1); mbar_init(acc_free + i, 4);
         }
+        for (int i = 0; i < NGK * 4; ++i) mbar_init(tok + i, 1);
         fence_barrier_init();
     }
     if (warp == 0) tmem_alloc<512>(tmem_slot);
@@ -281,6 +284,9 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         const uint64_t sl2 = pack2(sl, sl), l2e2 = pack2(kLog2e, kLog2e);
         const int sw = row & 7;
         int n = 0, un = 0, ia = 0;  // stage, unit and active-item counters
+        int ut = 0;                  // units seen (active or not): phase of the math-phase token
+        uint64_t* my_tok = tok + g * 4 + (warp & 3);
+        uint64_t* next_tok = tok + ((g + 1) % NGK) * 4 + (warp & 3);
         for (int il = 0; il < n_items; ++il) {
             const ItemK it = decode_itemk((int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
             const int r = it.r0 + g;
@@ -297,7 +303,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                     const uint8_t* brow = st + NGK * 2 * QS_BYTES + row * 128;
                     const float* ld = (const float*)(st + NGK * 2 * QS_BYTES + BIAS_BYTES) + g * 2 * BQS;
 #pragma unroll
-                    for (int hu = 0; hu < 2; ++hu, ++un) {
+                    for (int hu = 0; hu < 2; ++hu, ++un, ++ut) {
                         uint32_t bw[16];
 #pragma unroll
                         for (int j = 0; j < 4; ++j) {
@@ -306,16 +312,19 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                         }
                         mbar_wait(s_full + g, un & 1);
                         tc_fence_after();
-                        uint32_t pp[16], ds[16];
-#pragma unroll
-                        for (int ch = 0; ch < 2; ++ch) {
-                            uint32_t sr[16], dp[16];
-                            tmem_ld16(tS + ch * 16, sr);
-                            tmem_ld16(tDP + ch * 16, dp);
-                            tmem_ld_wait();
-                            dkdv_chunk(sr, dp, bw + ch * 8, ld + hu * BU + ch * 16, ld + BQS + hu * BU + ch * 16, sl2, l2e2, pp + ch * 8,
-                                       ds + ch * 8);
-                        }
+                        uint32_t sr[32], dp[32], pp[16], ds[16];
+                        tmem_ld32(tS, sr);
+                        tmem_ld32(tDP, dp);
+                        tmem_ld_wait();
+                        // The three groups' warps of one scheduler share its MUFU unit.  Left alone they run their exp phases
+                        // at the same time (each at a third of the rate) and then wait for their MMAs at the same time; the
+                        // token makes the exp phases take turns, so one group's MMA round trip hides under the others' math.
+                        if (g > 0 || ut > 0) mbar_wait(my_tok, (g > 0 ? ut : ut - 1) & 1);
+                        dkdv_chunk(*(const uint32_t(*)[16])&sr[0], *(const uint32_t(*)[16])&dp[0], bw, ld + hu * BU, ld + BQS + hu * BU, sl2,
+                                   l2e2, pp, ds);
+                        dkdv_chunk(*(const uint32_t(*)[16])&sr[16], *(const uint32_t(*)[16])&dp[16], bw + 8, ld + hu * BU + 16,
+                                   ld + BQS + hu * BU + 16, sl2, l2e2, pp + 8, ds + 8);
+                        if (lane == 0) mbar_arrive(next_tok);
                         if (!allkeep && !keep) {  // masked key: its whole row of P^T and dS^T is zero
 #pragma unroll
                             for (int e = 0; e < 16; ++e) { pp[e] = 0u; ds[e] = 0u; }
@@ -325,6 +334,12 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                         tmem_st_wait();
                         tc_fence_before();
                         warp_arrive(p_ready + g);
+                    }
+                } else {
+                    // a row group without a row in this item still passes the token on, once per unit
+                    for (int hu = 0; hu < 2; ++hu, ++ut) {
+                        if (g > 0 || ut > 0) mbar_wait(my_tok, (g > 0 ? ut : ut - 1) & 1);
+                        if (lane == 0) mbar_arrive(next_tok);
                     }
                 }
                 // my generic-proxy reads of the stage (bias^T, LSE / D) are complete before the producer may refill it
