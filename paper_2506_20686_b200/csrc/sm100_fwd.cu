@@ -32,6 +32,7 @@ constexpr int KT_BYTES = BK * DH * 2;      // 4 KB:  64 x 32 bf16
 constexpr int BIAS_BYTES = BQ * BK * 4;    // 32 KB: two [128 q][32 k] fp32 boxes (log2e * bias), SWIZZLE_128B
 constexpr float kLazy = 7.0f;              // lazy-rescale threshold on the running max (log2 units)
 constexpr int FWD_THREADS = (NG + 1) * 128;
+constexpr int kTokRelease = 24;            // pair index (of 32) of the exp loop at which the MUFU token moves on
 
 struct FwdSmem {
     static constexpr int q_off = 0;                                    // NG x 2 x Q tile
@@ -47,7 +48,8 @@ struct FwdSmem {
     static constexpr int b_consumed = b_s_full + NG;                   // [NG]
     static constexpr int b_p_ready = b_consumed + NG;                  // [NG]
     static constexpr int b_pv_done = b_p_ready + NG;                   // [NG]
-    static constexpr int n_bars = b_pv_done + NG;
+    static constexpr int b_tok = b_pv_done + NG;                       // [NG][4] exp-phase token of (group, scheduler quarter)
+    static constexpr int n_bars = b_tok + NG * 4;
     static constexpr int total = bar_off + n_bars * 8 + 16 + 1024;     // + tmem slot + alignment slack
 };
 
@@ -86,6 +88,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
     uint64_t* consumed = bars + L::b_consumed;
     uint64_t* p_ready = bars + L::b_p_ready;
     uint64_t* pv_done = bars + L::b_pv_done;
+    uint64_t* tok = bars + L::b_tok;
     uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5;
@@ -101,6 +104,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         for (int i = 0; i < NG; ++i) {
             mbar_init(s_full + i, 1); mbar_init(consumed + i, 4); mbar_init(p_ready + i, 4); mbar_init(pv_done + i, 1);
         }
+        for (int i = 0; i < NG * 4; ++i) mbar_init(tok + i, 1);
         fence_barrier_init();
     }
     if (warp == 0) tmem_alloc<512>(tmem_slot);
@@ -218,6 +222,8 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         const int NW = N / 64;  // mask words per row
         int bst = 0, bph = 0;
         int n = 0;
+        uint64_t* my_tok = tok + g * 4 + (warp & 3);
+        uint64_t* next_tok = tok + ((g + 1) % NG) * 4 + (warp & 3);
         for (int il = 0; il < n_items; ++il) {
             const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H);
             const int r = it.r4 + g;
@@ -278,9 +284,17 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 const float alpha = bump ? ex2(m_old - m_safe) : 1.0f;
                 const uint64_t mneg2 = pack2(-m_safe, -m_safe);
                 uint64_t lacc4[4] = {pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f), pack2(0.0f, 0.0f)};
+                // The four groups' warps of one scheduler share its MUFU unit, and one warp's exp loop saturates it.  Left
+                // alone the groups run their exp loops at the same time (each at a quarter of the rate) and then their
+                // score / max phases at the same time, with the unit idle; the token makes the exp loops take turns.
+                if (g > 0 || n > 0) mbar_wait(my_tok, (g > 0 ? n : n - 1) & 1);
                 uint32_t pk[BK / 2];
 #pragma unroll
                 for (int e = 0; e < BK / 2; ++e) {
+                    if (e == kTokRelease) {  // hand the token on a little early: the next warp's wake-up hides under my last exps
+                        __syncwarp();
+                        if ((tid & 31) == 0) mbar_arrive(next_tok);
+                    }
                     float a0, a1;
                     unpack2(add2(pack2(x[2 * e], x[2 * e + 1]), mneg2), a0, a1);
                     const float p0 = ex2(a0), p1 = ex2(a1);
