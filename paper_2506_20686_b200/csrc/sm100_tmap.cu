@@ -1,6 +1,8 @@
 // Host side of TMA: builds CUtensorMap descriptors with the driver's cuTensorMapEncodeTiled, resolved at run
 // time through the runtime API (no link-time dependency on libcuda).
 #include <mutex>
+#include <string.h>
+#include <unordered_map>
 
 #include "sm100_common.cuh"
 #include "tri_common.cuh"
@@ -25,9 +27,49 @@ EncodeTiledFn encode_fn() {
     return fn;
 }
 
+// Descriptor cache: a CUtensorMap is a pure function of (kind, base pointer, shape, variant, box), and a training loop
+// calls with the same buffers every step, so the driver's encode runs once per distinct key (bounded: flushed at 512 keys).
+struct TmapKey {
+    int kind;
+    const void* base;
+    int a, b, c, d, e, f;
+    bool operator==(const TmapKey& o) const { return memcmp(this, &o, sizeof(TmapKey)) == 0; }
+};
+struct TmapKeyHash {
+    size_t operator()(const TmapKey& k) const {
+        size_t h = (size_t)k.base * 1099511628211ull;
+        const int v[7] = {k.kind, k.a, k.b, k.c, k.d, k.e, k.f};
+        for (int x : v) h = (h ^ (size_t)x) * 1099511628211ull;
+        return h;
+    }
+};
+std::mutex g_tmap_mu;
+std::unordered_map<TmapKey, CUtensorMap, TmapKeyHash> g_tmap_cache;
+
+template <typename F>
+bool cached(const TmapKey& key, CUtensorMap* out, F&& encode) {
+    {
+        std::lock_guard<std::mutex> lock(g_tmap_mu);
+        auto it = g_tmap_cache.find(key);
+        if (it != g_tmap_cache.end()) {
+            *out = it->second;
+            return true;
+        }
+    }
+    if (!encode(out)) return false;
+    std::lock_guard<std::mutex> lock(g_tmap_mu);
+    if (g_tmap_cache.size() >= 512) g_tmap_cache.clear();
+    g_tmap_cache.emplace(key, *out);
+    return true;
+}
+
 }  // namespace
 
-bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d, int variant, int box_pos) {
+bool make_tmap_u(CUtensorMap* out_, const void* base, int B, int N, int H, int d, int variant, int box_pos) {
+    TmapKey key;
+    memset(&key, 0, sizeof(key));
+    key.kind = 0; key.base = base; key.a = B; key.b = N; key.c = H; key.d = d; key.e = variant; key.f = box_pos;
+    return cached(key, out_, [&](CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t es = 2;
@@ -45,9 +87,14 @@ bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
+    });
 }
 
-bool make_tmap_plane(CUtensorMap* out, const void* base, int BH, int N, int box_rows) {
+bool make_tmap_plane(CUtensorMap* out_, const void* base, int BH, int N, int box_rows) {
+    TmapKey key;
+    memset(&key, 0, sizeof(key));
+    key.kind = 1; key.base = base; key.a = BH; key.b = N; key.c = box_rows;
+    return cached(key, out_, [&](CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)BH};
@@ -58,9 +105,14 @@ bool make_tmap_plane(CUtensorMap* out, const void* base, int BH, int N, int box_
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
+    });
 }
 
-bool make_tmap_plane_f32(CUtensorMap* out, const void* base, int BH, int N, int box_rows) {
+bool make_tmap_plane_f32(CUtensorMap* out_, const void* base, int BH, int N, int box_rows) {
+    TmapKey key;
+    memset(&key, 0, sizeof(key));
+    key.kind = 2; key.base = base; key.a = BH; key.b = N; key.c = box_rows;
+    return cached(key, out_, [&](CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)BH};
@@ -71,6 +123,7 @@ bool make_tmap_plane_f32(CUtensorMap* out, const void* base, int BH, int N, int 
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
+    });
 }
 
 }  // namespace tri
