@@ -1,11 +1,11 @@
 // bf16 forward on tcgen05 / TMEM / TMA (sm_100a): flash-style online softmax, the [B,N,H,N,N] map never leaves
 // the SM (Listing 1, Sec. IV-A; gate, mask and 1/sqrt(d) from the task statement).
 //
-// Persistent, warp-specialised: one CTA per SM, 640 threads =
+// Persistent, warp-specialised: one CTA per SM, 768 threads =
 //   4 softmax warpgroups ("groups", 128 threads = 128 query rows = 128 TMEM lanes each) -- group g owns broadcast
 //     row 4*rq + g of the current work item (b, h, 128-query block qb, row quad rq) and walks its 64-key tiles;
-//   1 helper warpgroup: warp 16 = TMA producer, warps 17-18 = tcgen05.mma issuers (two groups each, one elected
-//     lane), warp 19 idle.
+//   2 helper warpgroups: warp 16 = TMA producer, warps 17-20 = one in-order tcgen05.mma issuer per group (one elected
+//     lane; they sleep in mbarrier.try_wait instead of polling), warps 21-23 idle.
 // Registers are moved from the helpers to the softmax warpgroups with setmaxnreg.  The four groups of a CTA work on
 // the same (b, h, qb), so one 128x64 bias tile (TMA, SWIZZLE_128B) serves four score tiles ("on-the-fly
 // broadcasting").  Per (group, tile) with TMEM columns [128g, 128g+128) = S 64 | P 32 | O 32:
@@ -31,7 +31,7 @@ constexpr int QT_BYTES = BQ * DH * 2;      // 8 KB: 128 x 32 bf16
 constexpr int KT_BYTES = BK * DH * 2;      // 4 KB:  64 x 32 bf16
 constexpr int BIAS_BYTES = BQ * BK * 4;    // 32 KB: two [128 q][32 k] fp32 boxes (log2e * bias), SWIZZLE_128B
 constexpr float kLazy = 7.0f;              // lazy-rescale threshold on the running max (log2 units)
-constexpr int FWD_THREADS = (NG + 1) * 128;
+constexpr int FWD_THREADS = (NG + 2) * 128;  // 4 softmax warpgroups + 2 helper warpgroups (TMA warp, 4 issuer warps)
 constexpr int kTokRelease = 24;            // pair index (of 32) of the exp loop at which the MUFU token moves on
 
 struct FwdSmem {
@@ -115,7 +115,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
 
     if (warp >= NG * 4) {
         // =============================== helper warpgroup ===============================
-        setmaxnreg_dec<40>();
+        setmaxnreg_dec<32>();
         if (warp == NG * 4) {
             // ---- TMA producer: bias tile of (item, kt) once, then (Q at kt = 0,) K, V of every group ----
             int kst = 0, kph = 0, bst = 0, bph = 0;
@@ -147,72 +147,53 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                     if (++bst == NB) { bst = 0; bph ^= 1; }
                 }
             }
-        } else if (warp == NG * 4 + 1 || warp == NG * 4 + 2) {
-            // ---- MMA issuers (warp-uniform control flow; one elected lane issues and commits) ----
-            // Warp 17 serves groups 0-1, warp 18 groups 2-3.  Each polls its groups: a group whose P(n) is ready gets
-            // O += P V; a group that has read S(n+1) out of TMEM gets S(n+2).  No group waits for another's epilogue.
-            constexpr int NGI = NG / 2;
-            const int g0 = (warp - (NG * 4 + 1)) * NGI;
+        } else if (warp <= NG * 4 + NG) {
+            // ---- tcgen05 issuer of group g (warp-uniform control flow; one elected lane issues and commits) ----
+            // In order, sleeping in mbarrier.try_wait: S(n) once the group has S(n-1) in registers and K(n) has landed, then
+            // O += P(n-1) V(n-1) once P(n-1) is stored -- the order in which the group raises those events.
+            const int g = warp - (NG * 4 + 1);
             constexpr uint32_t idescS = make_idesc(128, BK, false, false);
             constexpr uint32_t idescO = make_idesc(128, DH, false, true);
-            int s_n[NGI], s_st[NGI], s_kt[NGI], s_par[NGI];  // next S tile: index, ring stage, key tile, Q buffer
-            int p_n[NGI], p_st[NGI], p_kt[NGI];              // next P V tile
-#pragma unroll
-            for (int j = 0; j < NGI; ++j) { s_n[j] = s_st[j] = s_kt[j] = s_par[j] = 0; p_n[j] = p_st[j] = p_kt[j] = 0; }
-            const uint32_t qbase = smem_u32(sQ), kvbase = smem_u32(sKV);
-            int remaining = NGI * NT_all;
-            while (remaining > 0) {
-                // probe every barrier first (the probes are independent and overlap), then act
-                bool okS[NGI], okP[NGI];
-#pragma unroll
-                for (int j = 0; j < NGI; ++j) {
-                    const int g = g0 + j;
-                    const bool c = s_n[j] == 0 || mbar_test_wait(consumed + g, (s_n[j] - 1) & 1);
-                    const bool k = mbar_test_wait(kv_full + g * KV_ST + s_st[j], (s_n[j] / KV_ST) & 1);
-                    okS[j] = s_n[j] < NT_all && c && k;
-                    okP[j] = p_n[j] < NT_all && mbar_test_wait(p_ready + g, p_n[j] & 1);
+            const uint32_t qbase = smem_u32(sQ) + g * 2 * QT_BYTES, kvbase = smem_u32(sKV) + g * KV_ST * 2 * KT_BYTES;
+            const uint32_t tS = tmem + g * 128, tP = tS + 64, tO = tS + 96;
+            int st = 0, kt = 0, par = 0;     // ring stage, key tile and Q buffer of S(n)
+            int pst = 0, pkt = 0;            // ring stage and key tile of P(n-1) V(n-1)
+            for (int n = 0; n <= NT_all; ++n) {
+                if (n < NT_all) {
+                    mbar_wait(kv_full + g * KV_ST + st, (n / KV_ST) & 1);
+                    if (n > 0) mbar_wait(consumed + g, (n - 1) & 1);
+                    tc_fence_after();
+                    const uint64_t dq = make_desc_sw64(qbase + par * QT_BYTES);
+                    const uint64_t dk = make_desc_sw64(kvbase + st * 2 * KT_BYTES);
+                    if (elect_one()) {
+                        mma_ss(tS, dq, dk, idescS, 0);
+                        mma_ss(tS, dq + 2, dk + 2, idescS, 1);
+                        mma_commit(s_full + g);
+                    }
+                    __syncwarp();
+                    if (++st == KV_ST) st = 0;
+                    if (++kt == TPR) { kt = 0; par ^= 1; }
                 }
+                if (n > 0) {
+                    mbar_wait(p_ready + g, (n - 1) & 1);
+                    tc_fence_after();
+                    const uint64_t dv = make_desc_sw64(kvbase + pst * 2 * KT_BYTES + KT_BYTES);
+                    if (elect_one()) {
 #pragma unroll
-                for (int j = 0; j < NGI; ++j) {
-                    const int g = g0 + j;
-                    if (okP[j]) {  // O(g) += P(g, m) V(g, m)
-                        tc_fence_after();
-                        const uint64_t dv = make_desc_sw64(kvbase + (g * KV_ST + p_st[j]) * 2 * KT_BYTES + KT_BYTES);
-                        const uint32_t tP = tmem + g * 128 + 64, tO = tmem + g * 128 + 96;
-                        if (elect_one()) {
-#pragma unroll
-                            for (int ks = 0; ks < BK / 16; ++ks)
-                                mma_ts(tO, tP + ks * 8, dv + (uint64_t)ks * 64, idescO, (p_kt[j] > 0 || ks > 0) ? 1u : 0u);
-                            mma_commit(kv_free + g * KV_ST + p_st[j]);
-                            mma_commit(pv_done + g);
-                        }
-                        __syncwarp();
-                        ++p_n[j];
-                        --remaining;
-                        if (++p_st[j] == KV_ST) p_st[j] = 0;
-                        if (++p_kt[j] == TPR) p_kt[j] = 0;
+                        for (int ks = 0; ks < BK / 16; ++ks)
+                            mma_ts(tO, tP + ks * 8, dv + (uint64_t)ks * 64, idescO, (pkt > 0 || ks > 0) ? 1u : 0u);
+                        mma_commit(kv_free + g * KV_ST + pst);
+                        mma_commit(pv_done + g);
                     }
-                    if (okS[j]) {  // S(g, m): S columns free (tile m-1 read out), K (and Q) of tile m in shared memory
-                        tc_fence_after();
-                        const uint64_t dq = make_desc_sw64(qbase + (g * 2 + s_par[j]) * QT_BYTES);
-                        const uint64_t dk = make_desc_sw64(kvbase + (g * KV_ST + s_st[j]) * 2 * KT_BYTES);
-                        const uint32_t tS = tmem + g * 128;
-                        if (elect_one()) {
-                            mma_ss(tS, dq, dk, idescS, 0);
-                            mma_ss(tS, dq + 2, dk + 2, idescS, 1);
-                            mma_commit(s_full + g);
-                        }
-                        __syncwarp();
-                        ++s_n[j];
-                        if (++s_st[j] == KV_ST) s_st[j] = 0;
-                        if (++s_kt[j] == TPR) { s_kt[j] = 0; s_par[j] ^= 1; }
-                    }
+                    __syncwarp();
+                    if (++pst == KV_ST) pst = 0;
+                    if (++pkt == TPR) pkt = 0;
                 }
             }
         }
     } else {
         // =============================== softmax groups ===============================
-        setmaxnreg_inc<104>();  // 512 x 104 + 128 x 40 <= 640 x 96 (the launch allocation)
+        setmaxnreg_inc<104>();  // 512 x 104 + 256 x 32 = 768 x 80 (the launch allocation)
         const int g = warp >> 2;
         const int row = tid & 127;                                  // query row inside the block = TMEM lane
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
