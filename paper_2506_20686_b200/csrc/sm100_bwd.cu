@@ -6,6 +6,8 @@
 //            dV += P^T dA, dK += dS^T Q
 //   dqdb     (sm100_dqdb.cu) dQ and dBias from one recomputation, tile-stationary, cluster reduce of dQ
 //   reduce   level 2 of the dBias reduction: adds the row-split partial planes in ascending order
+#include <mutex>
+
 #include "sm100_common.cuh"
 #include "tri_common.cuh"
 
@@ -92,6 +94,27 @@ BwdWs bwd_ws_layout(const Problem& p) {
     w.total = o;
     return w;
 }
+// one side stream + fork / join events per device (created on first use, never destroyed)
+struct SideStream {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+    bool ready = false;
+};
+std::mutex g_side_mu;
+SideStream g_side[64];
+SideStream* side_stream() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(g_side_mu);
+    SideStream& s = g_side[dev];
+    if (!s.ready) {
+        if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        s.ready = true;
+    }
+    return &s;
+}
 template <typename K>
 tri_status set_smem(K kern, int bytes) {
     TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
@@ -126,21 +149,48 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
         if ((s = sm100_pack_mask(p, mask, maskbits, st)) != TRI_OK) return s;
         TRI_LAUNCH_CHECK("pack_mask_kernel");
     }
-    // stage 1: dK, dV (key-stationary)
-    if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, LSE, Dws, (float*)((char*)ws + w.nl_off),
-                                (float*)((char*)ws + w.nd_off), dK, dV, st)) != TRI_OK)
-        return s;
-    // stage 2, fused: dQ and dBias from one recomputation of P / dS (cluster over the key tiles of a query block)
-    float* planes = (float*)((char*)ws + w.planes_off);
-    int Gs = 1, C2 = 0, grid2 = 0;
-    if (!sm100_dqdb_plan(p, &C2, &Gs, &grid2)) return cuda_fail(cudaErrorLaunchFailure, "sm100_dqdb_plan: no resident cluster of the needed size");
+    float* NL = (float*)((char*)ws + w.nl_off);
+    float* ND = (float*)((char*)ws + w.nd_off);
+    if ((s = sm100_lse_prep(p, LSE, Dws, NL, ND, st)) != TRI_OK) return s;
     float* biasL = (float*)((char*)ws + w.biasl_off);
     {
         const bool tr = p.variant == TRI_ENDING;
         if ((s = sm100_bias_planes(bias, tr ? nullptr : biasL, tr ? biasL : nullptr, p.B * p.H, p.N, kLog2e, st)) != TRI_OK) return s;
         TRI_LAUNCH_CHECK("bias_planes_kernel");
     }
+    // Stage 2 (dQ + dBias, one recomputation of P / dS) runs as clusters and leaves some SMs empty (132 of 148 at N = 768:
+    // cudaOccupancyMaxActiveClusters).  Stage 1 (dK, dV) is independent of it, so a first slice of stage 1's work items runs
+    // on those SMs at the same time, on a library-owned side stream forked from and joined back into `st` with events;
+    // the rest of stage 1 follows on all SMs.
+    float* planes = (float*)((char*)ws + w.planes_off);
+    int Gs = 1, C2 = 0, grid2 = 0;
+    if (!sm100_dqdb_plan(p, &C2, &Gs, &grid2)) return cuda_fail(cudaErrorLaunchFailure, "sm100_dqdb_plan: no resident cluster of the needed size");
+    const long long items1 = sm100_dkdv2_items(p);
+    const int sms = sm100_sm_count();
+    const int spare = sms - grid2;
+    long long itemsA = 0;
+    SideStream* side = nullptr;
+    if (spare >= 4 && items1 > 4 * sms) {
+        // the spare SMs work for about the duration of stage 2, which is ~1.4x stage 1's on the whole chip
+        itemsA = (long long)((double)items1 * spare / sms * 1.4);
+        side = side_stream();
+        if (!side) itemsA = 0;
+    }
+    if (itemsA > 0) {
+        TRI_CUDA_CHECK(cudaEventRecord(side->fork, st));
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(side->stream, side->fork, 0));
+    }
     if ((s = sm100_dqdb_launch(p, C2, Gs, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dBias, planes, st)) != TRI_OK) return s;
+    if (itemsA > 0) {
+        if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, NL, ND, dK, dV, 0, itemsA, spare, "sm100_dkdv_kernel(side)",
+                                    side->stream)) != TRI_OK)
+            return s;
+        TRI_CUDA_CHECK(cudaEventRecord(side->join, side->stream));
+    }
+    if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, NL, ND, dK, dV, itemsA, items1 - itemsA, sms, "sm100_dkdv_kernel", st)) !=
+        TRI_OK)
+        return s;
+    if (itemsA > 0) TRI_CUDA_CHECK(cudaStreamWaitEvent(st, side->join, 0));
     if (Gs > 1) {
         {
             ProfScope ps("sm100_dbias_reduce_kernel", st);

@@ -102,7 +102,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                    const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                    const __grid_constant__ CUtensorMap tmBiasKQ, Problem p, const unsigned long long* __restrict__ maskbits,
                    const float* __restrict__ NL, const float* __restrict__ ND, __nv_bfloat16* __restrict__ dK,
-                   __nv_bfloat16* __restrict__ dV, int total_items) {
+                   __nv_bfloat16* __restrict__ dV, int item_begin, int total_items) {
     using L = DkdvSmem;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -150,7 +150,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             // ---- TMA producer ----
             int n = 0;  // stage counter over the CTA's life
             for (int il = 0; il < n_items; ++il) {
-                const ItemK it = decode_itemk((int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
+                const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
                 const int bh = it.b * p.H + it.h;
                 const int nr = min(NGK, N - it.r0);  // active rows of the item
                 if (il > 0) mbar_wait(kv_free, (il - 1) & 1);
@@ -192,7 +192,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             int un = 0;  // unit counter (barrier phases of s_full / p_ready)
             int ia = 0;  // rows this group has processed (barrier phases of acc_full / acc_free)
             for (int il = 0; il < n_items; ++il) {
-                const ItemK it = decode_itemk((int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
+                const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
                 const bool active = it.r0 + g < N;
                 mbar_wait(kv_full, il & 1);
                 tc_fence_after();
@@ -288,7 +288,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         uint64_t* my_tok = tok + g * 4 + (warp & 3);
         uint64_t* next_tok = tok + ((g + 1) % NGK) * 4 + (warp & 3);
         for (int il = 0; il < n_items; ++il) {
-            const ItemK it = decode_itemk((int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
+            const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
             const int r = it.r0 + g;
             const bool active = r < N;
             bool keep = true;
@@ -402,28 +402,34 @@ __global__ void __launch_bounds__(256) lse_prep_kernel(const float* __restrict__
 
 size_t sm100_dkdv2_aux_bytes(const Problem& p) { return align_up((size_t)p.B * p.N * p.H * p.N * 4, 256); }
 
-tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, const void* K, const void* V, const void* bias_kq,
-                              const unsigned long long* maskbits, const float* LSE, const float* Dws, float* NL, float* ND,
-                              void* dK, void* dV, cudaStream_t st) {
+long long sm100_dkdv2_items(const Problem& p) { return (long long)p.B * p.H * (p.N / BKEY) * ((p.N + NGK - 1) / NGK); }
+
+tri_status sm100_lse_prep(const Problem& p, const float* LSE, const float* Dws, float* NL, float* ND, cudaStream_t st) {
+    const long long total = (long long)p.B * p.N * p.H * p.N;
     {
-        const long long total = (long long)p.B * p.N * p.H * p.N;
         ProfScope ps("lse_prep_kernel", st);
         lse_prep_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(LSE, Dws, NL, ND, p);
     }
     TRI_LAUNCH_CHECK("lse_prep_kernel");
+    return TRI_OK;
+}
+
+// work items [item_begin, item_begin + item_count) on at most max_ctas persistent CTAs
+tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, const void* K, const void* V, const void* bias_kq,
+                              const unsigned long long* maskbits, const float* NL, const float* ND, void* dK, void* dV,
+                              long long item_begin, long long item_count, int max_ctas, const char* prof_name, cudaStream_t st) {
+    if (item_count <= 0) return TRI_OK;
     CUtensorMap tQ, tA, tK, tV, tB;
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQS) || !make_tmap_u(&tA, dA, p.B, p.N, p.H, p.d, p.variant, BQS) ||
         !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BKEY) || !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BKEY) ||
         !make_tmap_plane(&tB, bias_kq, p.B * p.H, p.N, BKEY))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_dkdv2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DkdvSmem::total));
-    const long long items = (long long)p.B * p.H * (p.N / BKEY) * ((p.N + NGK - 1) / NGK);
-    const int sms = sm100_sm_count();
-    const int grid = (int)(items < sms ? items : sms);
+    const int grid = (int)(item_count < max_ctas ? item_count : max_ctas);
     {
-        ProfScope ps("sm100_dkdv_kernel", st);
+        ProfScope ps(prof_name, st);
         sm100_dkdv2_kernel<<<grid, DKDV_THREADS, DkdvSmem::total, st>>>(tQ, tA, tK, tV, tB, p, maskbits, NL, ND, (__nv_bfloat16*)dK,
-                                                                       (__nv_bfloat16*)dV, (int)items);
+                                                                       (__nv_bfloat16*)dV, (int)item_begin, (int)item_count);
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
     return TRI_OK;

@@ -91,11 +91,14 @@ tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int 
 // keep flags -> one 64-bit word per (b, row, 64-key tile), rows / keys in the variant's sense
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st);
 size_t sm100_maskbits_bytes(const Problem& p);
-// dK / dV stage (sm100_dkdv.cu): NL / ND are fp32 [B,N,H,N] scratch arrays of sm100_dkdv2_aux_bytes() each
+// dK / dV stage (sm100_dkdv.cu): NL / ND are fp32 [B,N,H,N] scratch arrays of sm100_dkdv2_aux_bytes() each, filled by
+// sm100_lse_prep; a launch covers work items [item_begin, item_begin + item_count) of sm100_dkdv2_items() on <= max_ctas CTAs
 size_t sm100_dkdv2_aux_bytes(const Problem& p);
+long long sm100_dkdv2_items(const Problem& p);
+tri_status sm100_lse_prep(const Problem& p, const float* LSE, const float* Dws, float* NL, float* ND, cudaStream_t st);
 tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, const void* K, const void* V, const void* bias_kq,
-                              const unsigned long long* maskbits, const float* LSE, const float* Dws, float* NL, float* ND,
-                              void* dK, void* dV, cudaStream_t st);
+                              const unsigned long long* maskbits, const float* NL, const float* ND, void* dK, void* dV,
+                              long long item_begin, long long item_count, int max_ctas, const char* prof_name, cudaStream_t st);
 // fused dQ + dBias stage (sm100_dqdb.cu): cluster size (0 = shape not covered), row split, persistent grid, launch
 int sm100_dqdb_cluster(int N);
 constexpr int kDqdbMaxSplit = 8;  // the workspace holds this many partial dBias planes
