@@ -34,7 +34,10 @@
  *   - Every tensor pointer of tri_attn_fwd / tri_attn_bwd is a caller-owned DEVICE pointer, 16-byte
  *     aligned.  The library never allocates or frees device memory and never synchronises the
  *     device: all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the
- *     legacy default stream).  Scratch space comes from `workspace` (device, 256-byte aligned, at
+ *     legacy default stream) -- or, for kernels that may overlap (tri_attn_bwd runs a slice of its
+ *     dK/dV stage beside its dQ/dBias stage; tri_attn_step_host overlaps copies and compute), on
+ *     library-owned side streams that are forked from and joined back into `cuda_stream` with
+ *     events inside the call, so to the caller each call is still one unit of work on `cuda_stream`.  Scratch space comes from `workspace` (device, 256-byte aligned, at
  *     least *_workspace_bytes() bytes, contents undefined on entry and exit).  workspace_bytes is
  *     O(B*H*N^2*d) (the backward keeps one dA = dO (.) sigmoid(G) tensor there); nothing of size
  *     B*H*N^3 exists anywhere.
