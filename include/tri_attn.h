@@ -106,6 +106,28 @@ TRI_API tri_status tri_attn_bwd(const void* dO,
                         int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
                         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Decoupled row count ("EvoAttention" with rows != N, e.g. MSA-row attention with pair bias, or a
+ * chunk of the rows of a pair tensor): R independent broadcast rows, each attending over N positions with the shared
+ * bias[b,h,j,k].  Starting-node index convention only:
+ *     Q,K,V,G,O,dO,dQ,dK,dV,dG : [B, R, H, N, d]     mask : [B, R, N] (or NULL)     LSE : [B, R, H, N]
+ *     bias, dBias              : [B, H, N, N]        dBias[b,h,j,k] = sum over the R rows of dS
+ * Runs on the tensor-core kernels only: bf16, d == 32, N % 128 == 0, N <= 2048, R % 4 == 0; anything else returns
+ * TRI_ERR_UNSUPPORTED (workspace queries return 0).  tri_attn_fwd / tri_attn_bwd are the R == N case. */
+TRI_API size_t tri_attn_rows_fwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype);
+TRI_API size_t tri_attn_rows_bwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype);
+TRI_API tri_status tri_attn_rows_fwd(const void* Q, const void* K, const void* V, const void* G,
+                             const void* bias, const unsigned char* mask /* NULL = no mask */,
+                             void* O, float* LSE,
+                             int B, int R, int N, int H, int d, tri_dtype dtype,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+TRI_API tri_status tri_attn_rows_bwd(const void* dO,
+                             const void* Q, const void* K, const void* V, const void* G,
+                             const void* bias, const unsigned char* mask,
+                             const void* O, const float* LSE,
+                             void* dQ, void* dK, void* dV, void* dG, float* dBias,
+                             int B, int R, int N, int H, int d, tri_dtype dtype,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* End-to-end step on HOST buffers: H2D(Q,K,V,G,bias,mask,dO) -> fwd -> bwd -> D2H(O,LSE,dQ,dK,dV,
  * dG,dBias).  `arena` is a caller-owned device buffer of tri_attn_step_host_arena_bytes() bytes. */
 TRI_API size_t tri_attn_step_host_arena_bytes(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);

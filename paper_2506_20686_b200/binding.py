@@ -26,6 +26,10 @@ SIGNATURES = {
     "tri_attn_bwd_workspace_bytes": (_sz, [_i] * 6),
     "tri_attn_fwd": (_i, [_vp] * 8 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_bwd": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
+    "tri_attn_rows_fwd_workspace_bytes": (_sz, [_i] * 6),
+    "tri_attn_rows_bwd_workspace_bytes": (_sz, [_i] * 6),
+    "tri_attn_rows_fwd": (_i, [_vp] * 8 + [_i] * 6 + [_vp, _sz, _vp]),
+    "tri_attn_rows_bwd": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_step_host_arena_bytes": (_sz, [_i] * 6),
     "tri_attn_step_host": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_uses_tensor_cores": (_i, [_i] * 6),
@@ -188,6 +192,71 @@ def tri_attn_bwd(dO, Q, K, V, G, bias, mask, O, LSE, variant=STARTING, out=None,
         _check(lib.tri_attn_bwd(_ptr(dO), _ptr(Q), _ptr(K), _ptr(V), _ptr(G), _ptr(bias), _ptr(mask), _ptr(O),
                                 _ptr(LSE), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(dG), _ptr(dBias),
                                 B, N, H, d, variant, code, _ptr(ws), ws.numel(), stream))
+    return dQ, dK, dV, dG, dBias
+
+
+def rows_fwd_workspace_bytes(B, R, N, H, d, dtype_code) -> int:
+    return int(load().tri_attn_rows_fwd_workspace_bytes(B, R, N, H, d, dtype_code))
+
+
+def rows_bwd_workspace_bytes(B, R, N, H, d, dtype_code) -> int:
+    return int(load().tri_attn_rows_bwd_workspace_bytes(B, R, N, H, d, dtype_code))
+
+
+def tri_attn_rows_fwd(Q, K, V, G, bias, mask=None, O=None, LSE=None, workspace=None):
+    """O, LSE = forward with a decoupled row count: Q,K,V,G [B,R,H,N,d], bias [B,H,N,N], mask [B,R,N] (starting node)."""
+    lib = load()
+    if not Q.is_cuda:
+        raise TriAttnError("tri_attn_rows_fwd needs CUDA tensors (there is no CPU path)")
+    B, R, H, N, d = Q.shape
+    dt, dev = Q.dtype, Q.device
+    for t, n in ((Q, "Q"), (K, "K"), (V, "V"), (G, "G")):
+        _chk(t, Q.shape, dt, n, dev)
+    _chk(bias, (B, H, N, N), dt, "bias", dev)
+    _chk(mask, (B, R, N), torch.uint8, "mask", dev)
+    if O is None:
+        O = torch.empty_like(Q)
+    if LSE is None:
+        LSE = torch.empty((B, R, H, N), dtype=torch.float32, device=dev)
+    _chk(O, Q.shape, dt, "O", dev)
+    _chk(LSE, (B, R, H, N), torch.float32, "LSE", dev)
+    code = _dtype_code(Q)
+    need = rows_fwd_workspace_bytes(B, R, N, H, d, code)
+    ws = _workspace(need, dev, workspace)
+    with torch.cuda.device(dev):
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(lib.tri_attn_rows_fwd(_ptr(Q), _ptr(K), _ptr(V), _ptr(G), _ptr(bias), _ptr(mask), _ptr(O), _ptr(LSE),
+                                     B, R, N, H, d, code, _ptr(ws), ws.numel(), stream))
+    return O, LSE
+
+
+def tri_attn_rows_bwd(dO, Q, K, V, G, bias, mask, O, LSE, out=None, workspace=None):
+    """dQ, dK, dV, dG, dBias = backward of tri_attn_rows_fwd; dBias [B,H,N,N] fp32 sums over the R rows."""
+    lib = load()
+    if not Q.is_cuda:
+        raise TriAttnError("tri_attn_rows_bwd needs CUDA tensors (there is no CPU path)")
+    B, R, H, N, d = Q.shape
+    dt, dev = Q.dtype, Q.device
+    for t, n in ((dO, "dO"), (Q, "Q"), (K, "K"), (V, "V"), (G, "G"), (O, "O")):
+        _chk(t, Q.shape, dt, n, dev)
+    _chk(bias, (B, H, N, N), dt, "bias", dev)
+    _chk(mask, (B, R, N), torch.uint8, "mask", dev)
+    _chk(LSE, (B, R, H, N), torch.float32, "LSE", dev)
+    if out is None:
+        out = tuple(torch.empty_like(Q) for _ in range(4)) + (
+            torch.empty((B, H, N, N), dtype=torch.float32, device=dev),)
+    dQ, dK, dV, dG, dBias = out
+    for t, n in ((dQ, "dQ"), (dK, "dK"), (dV, "dV"), (dG, "dG")):
+        _chk(t, Q.shape, dt, n, dev)
+    _chk(dBias, (B, H, N, N), torch.float32, "dBias", dev)
+    code = _dtype_code(Q)
+    need = rows_bwd_workspace_bytes(B, R, N, H, d, code)
+    ws = _workspace(need, dev, workspace)
+    with torch.cuda.device(dev):
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(lib.tri_attn_rows_bwd(_ptr(dO), _ptr(Q), _ptr(K), _ptr(V), _ptr(G), _ptr(bias), _ptr(mask), _ptr(O),
+                                     _ptr(LSE), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(dG), _ptr(dBias),
+                                     B, R, N, H, d, code, _ptr(ws), ws.numel(), stream))
     return dQ, dK, dV, dG, dBias
 
 

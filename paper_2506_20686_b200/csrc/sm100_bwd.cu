@@ -81,8 +81,8 @@ struct BwdWs {
 BwdWs bwd_ws_layout(const Problem& p) {
     BwdWs w;
     size_t o = 0;
-    w.d_off = o; o += align_up((size_t)p.B * p.N * p.H * p.N * sizeof(float), 256);          // D = rowsum(dO . O)
-    w.da_off = o; o += align_up((size_t)p.B * p.N * p.H * p.N * p.d * 2, 256);               // dA = dO . sigmoid(G)
+    w.d_off = o; o += align_up((size_t)p.B * p.R * p.H * p.N * sizeof(float), 256);          // D = rowsum(dO . O)
+    w.da_off = o; o += align_up((size_t)p.B * p.R * p.H * p.N * p.d * 2, 256);               // dA = dO . sigmoid(G)
     w.biast_off = o; o += align_up((size_t)p.B * p.H * p.N * p.N * 2, 256);                  // bias^T, bf16 (dkdv)
     w.biasl_off = o; o += align_up((size_t)p.B * p.H * p.N * p.N * 4, 256);                  // log2e * bias[q][k], fp32 (dqdb)
     w.mask_off = o; o += sm100_maskbits_bytes(p);
@@ -131,7 +131,7 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     float* Dws = (float*)((char*)ws + w.d_off);
     void* dA = (char*)ws + w.da_off;
     void* biasT = (char*)ws + w.biast_off;
-    const long long rows = (long long)p.B * p.N * p.H * p.N;
+    const long long rows = (long long)p.B * p.R * p.H * p.N;
     {
         ProfScope ps("sm100_bwd_pre_kernel", st);
         sm100_bwd_pre_kernel<<<(unsigned)((rows * 4 + 255) / 256), 256, 0, st>>>(rows, (const uint4*)dO, (const uint4*)O,

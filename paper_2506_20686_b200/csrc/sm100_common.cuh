@@ -285,7 +285,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 // ---- host: tensor maps (sm100_tmap.cu) ---------------------------------------------------------------
 // 5-D map over a [B,N,H,N,d] bf16 tensor with dims ordered (d, pos, row, h, b) for the given variant; box =
 // {d, box_pos, 1, 1, 1}, SWIZZLE_64B (d = 32 -> 64-byte rows).
-bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d, int variant, int box_pos);
+bool make_tmap_u(CUtensorMap* out, const void* base, int B, int N, int H, int d, int variant, int box_pos, int rows = -1);
 // 3-D map over a [BH, N, N] bf16 plane stack, dims (col, row, bh); box = {64, box_rows, 1}, SWIZZLE_128B.
 bool make_tmap_plane(CUtensorMap* out, const void* base, int BH, int N, int box_rows);
 // 3-D map over a [BH, N, N] fp32 plane stack, dims (col, row, bh); box = {32, box_rows, 1} (128-byte rows), SWIZZLE_128B.

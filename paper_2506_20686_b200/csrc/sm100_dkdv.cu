@@ -122,7 +122,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int N = p.N, NW = N / 64;
-    const int NT3 = (N + NGK - 1) / NGK;  // row triples (the last one may be partial)
+    const int NT3 = (p.R + NGK - 1) / NGK;  // row triples (the last one may be partial)
     const int NS = N / BQS;               // ring stages per row
     const int n_items = (total_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
 
@@ -152,7 +152,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             for (int il = 0; il < n_items; ++il) {
                 const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
                 const int bh = it.b * p.H + it.h;
-                const int nr = min(NGK, N - it.r0);  // active rows of the item
+                const int nr = min(NGK, p.R - it.r0);  // active rows of the item
                 if (il > 0) mbar_wait(kv_free, (il - 1) & 1);
                 if (elect_one()) {
                     mbar_expect_tx(kv_full, nr * 2 * KV_BYTES);
@@ -171,7 +171,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                         for (int g = 0; g < nr; ++g) {
                             tma_load_5d(st + g * 2 * QS_BYTES, &tmQ, full + s, 0, sq * BQS, it.r0 + g, it.h, it.b);
                             tma_load_5d(st + g * 2 * QS_BYTES + QS_BYTES, &tmA, full + s, 0, sq * BQS, it.r0 + g, it.h, it.b);
-                            const long long o = (((long long)it.b * N + it.r0 + g) * p.H + it.h) * N + sq * BQS;
+                            const long long o = (((long long)it.b * p.R + it.r0 + g) * p.H + it.h) * N + sq * BQS;
                             float* ld = (float*)(st + NGK * 2 * QS_BYTES + BIAS_BYTES) + g * 2 * BQS;
                             bulk_load(ld, NL + o, BQS * 4, full + s);
                             bulk_load(ld + BQS, ND + o, BQS * 4, full + s);
@@ -193,7 +193,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             int ia = 0;  // rows this group has processed (barrier phases of acc_full / acc_free)
             for (int il = 0; il < n_items; ++il) {
                 const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
-                const bool active = it.r0 + g < N;
+                const bool active = it.r0 + g < p.R;
                 mbar_wait(kv_full, il & 1);
                 tc_fence_after();
                 if (active) {
@@ -290,10 +290,10 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         for (int il = 0; il < n_items; ++il) {
             const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
             const int r = it.r0 + g;
-            const bool active = r < N;
+            const bool active = r < p.R;
             bool keep = true;
             if (active && maskbits)
-                keep = (ldg_u64(maskbits + ((long long)it.b * N + r) * NW + (it.k0 + row) / 64) >> ((it.k0 + row) & 63)) & 1ull;
+                keep = (ldg_u64(maskbits + ((long long)it.b * p.R + r) * NW + (it.k0 + row) / 64) >> ((it.k0 + row) & 63)) & 1ull;
             const bool allkeep = __all_sync(0xffffffffu, keep);
             for (int sq = 0; sq < NS; ++sq, ++n) {
                 const int s = n % NSTG;
@@ -383,16 +383,16 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
 // 32 queries are contiguous for both variants
 __global__ void __launch_bounds__(256) lse_prep_kernel(const float* __restrict__ LSE, const float* __restrict__ Dws,
                                                        float* __restrict__ NL, float* __restrict__ ND, Problem p) {
-    const long long total = (long long)p.B * p.N * p.H * p.N;
+    const long long total = (long long)p.B * p.R * p.H * p.N;
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
     const int q = (int)(i % p.N);
     long long t = i / p.N;
     const int h = (int)(t % p.H);
     t /= p.H;
-    const int r = (int)(t % p.N);
-    const int b = (int)(t / p.N);
-    const long long src = (long long)b * p.N * p.H * p.N + (long long)h * p.N + (long long)r * p.lR + (long long)q * p.lQ;
+    const int r = (int)(t % p.R);
+    const int b = (int)(t / p.R);
+    const long long src = (long long)b * p.lB + (long long)h * p.N + (long long)r * p.lR + (long long)q * p.lQ;
     const float l = __ldg(LSE + src);
     NL[i] = l == -INFINITY ? -INFINITY : -l * kLog2e;
     ND[i] = -__ldg(Dws + src);
@@ -400,12 +400,12 @@ __global__ void __launch_bounds__(256) lse_prep_kernel(const float* __restrict__
 
 }  // namespace
 
-size_t sm100_dkdv2_aux_bytes(const Problem& p) { return align_up((size_t)p.B * p.N * p.H * p.N * 4, 256); }
+size_t sm100_dkdv2_aux_bytes(const Problem& p) { return align_up((size_t)p.B * p.R * p.H * p.N * 4, 256); }
 
-long long sm100_dkdv2_items(const Problem& p) { return (long long)p.B * p.H * (p.N / BKEY) * ((p.N + NGK - 1) / NGK); }
+long long sm100_dkdv2_items(const Problem& p) { return (long long)p.B * p.H * (p.N / BKEY) * ((p.R + NGK - 1) / NGK); }
 
 tri_status sm100_lse_prep(const Problem& p, const float* LSE, const float* Dws, float* NL, float* ND, cudaStream_t st) {
-    const long long total = (long long)p.B * p.N * p.H * p.N;
+    const long long total = (long long)p.B * p.R * p.H * p.N;
     {
         ProfScope ps("lse_prep_kernel", st);
         lse_prep_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(LSE, Dws, NL, ND, p);
@@ -420,8 +420,8 @@ tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, c
                               long long item_begin, long long item_count, int max_ctas, const char* prof_name, cudaStream_t st) {
     if (item_count <= 0) return TRI_OK;
     CUtensorMap tQ, tA, tK, tV, tB;
-    if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQS) || !make_tmap_u(&tA, dA, p.B, p.N, p.H, p.d, p.variant, BQS) ||
-        !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BKEY) || !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BKEY) ||
+    if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQS, p.R) || !make_tmap_u(&tA, dA, p.B, p.N, p.H, p.d, p.variant, BQS, p.R) ||
+        !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BKEY, p.R) || !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BKEY, p.R) ||
         !make_tmap_plane(&tB, bias_kq, p.B * p.H, p.N, BKEY))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_dkdv2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DkdvSmem::total));

@@ -176,7 +176,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int nt = base_t + (c < rem_t ? 1 : 0);
     const int t0 = c * base_t + (c < rem_t ? c : rem_t);
     const int k0 = t0 * BK;
-    const int NR = N / G;  // broadcast rows per work item
+    const int NR = p.R / G;  // broadcast rows per work item
     const int cid = (int)blockIdx.x / C, ncl = (int)gridDim.x / C;
     const int n_my = (n_items - cid + ncl - 1) / ncl;
     const int NRtot = n_my * NR;
@@ -331,10 +331,10 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             int n = 0;
             for (int il = 0; il < n_my; ++il) {
                 const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
-                const float* lp = LSE + (long long)it.b * N * p.H * N + (long long)it.h * N + (long long)(it.q0 + row) * p.lQ +
+                const float* lp = LSE + (long long)it.b * p.lB + (long long)it.h * N + (long long)(it.q0 + row) * p.lQ +
                                   (long long)it.rb * p.lR;
                 const float* dp_ = Dws + (lp - LSE);
-                const unsigned long long* mp = maskbits ? maskbits + ((long long)it.b * N + it.rb) * NW + tile : nullptr;
+                const unsigned long long* mp = maskbits ? maskbits + ((long long)it.b * p.R + it.rb) * NW + tile : nullptr;
                 float lse_n = __ldg(lp), dd_n = __ldg(dp_);
                 uint64_t mb_n = mp ? ldg_u64(mp) : ~0ull;
                 // my row of the bias tile -> registers for the whole item; the shared buffer goes back to the producer
@@ -519,9 +519,9 @@ bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
     int bestG = 1;
     double best = 1e30;
     for (int G = 1; G <= kDqdbMaxSplit; ++G) {
-        if (p.N % G) continue;
+        if (p.R % G) continue;
         const double waves = (double)((base * G + ncl - 1) / ncl);
-        const double cost = waves * (p.N / G + 12);  // + per-item fill / drain / dBias flush in row units
+        const double cost = waves * (p.R / G + 12);  // + per-item fill / drain / dBias flush in row units
         if (cost < best * 0.99) { best = cost; bestG = G; }
     }
     const long long items = base * bestG;
@@ -535,8 +535,8 @@ tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const voi
                              void* dQ, float* dBias, float* planes, cudaStream_t st) {
     const int kbox = p.N < NGB * BK ? p.N : NGB * BK;
     CUtensorMap tQ, tA, tK, tV, tB;
-    if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tA, dA, p.B, p.N, p.H, p.d, p.variant, BQ) ||
-        !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, kbox) || !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, kbox) ||
+    if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ, p.R) || !make_tmap_u(&tA, dA, p.B, p.N, p.H, p.d, p.variant, BQ, p.R) ||
+        !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, kbox, p.R) || !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, kbox, p.R) ||
         !make_tmap_plane_f32(&tB, biasL_qk, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     cudaLaunchConfig_t cfg = {};

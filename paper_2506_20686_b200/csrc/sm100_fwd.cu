@@ -56,8 +56,8 @@ struct FwdSmem {
 struct Item { int b, h, q0, r4; };
 // row quad fastest (measured: query block fastest halves the K / V re-reads from HBM but is 4 % slower at cfg5, where
 // the ending-node rows are 64-byte neighbours in memory and concurrent quads share DRAM pages)
-__device__ __forceinline__ Item decode_item(int item, int N, int H) {
-    const int NRQ = N / NG, NQB = N / BQ;
+__device__ __forceinline__ Item decode_item(int item, int N, int H, int R) {
+    const int NRQ = R / NG, NQB = N / BQ;
     Item it;
     it.r4 = (item % NRQ) * NG;
     int t = item / NRQ;
@@ -120,7 +120,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
             // ---- TMA producer: bias tile of (item, kt) once, then (Q at kt = 0,) K, V of every group ----
             int kst = 0, kph = 0, bst = 0, bph = 0;
             for (int il = 0; il < n_items; ++il) {
-                const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H);
+                const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
                 const int bh = it.b * p.H + it.h;
                 for (int kt = 0; kt < TPR; ++kt) {
                     mbar_wait(bias_free + bst, bph ^ 1);
@@ -206,9 +206,9 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         uint64_t* my_tok = tok + g * 4 + (warp & 3);
         uint64_t* next_tok = tok + ((g + 1) % NG) * 4 + (warp & 3);
         for (int il = 0; il < n_items; ++il) {
-            const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H);
+            const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
             const int r = it.r4 + g;
-            const unsigned long long* mrow = maskbits ? maskbits + ((long long)it.b * N + r) * NW : nullptr;
+            const unsigned long long* mrow = maskbits ? maskbits + ((long long)it.b * p.R + r) * NW : nullptr;
             uint64_t mb_next = mrow ? ldg_u64(mrow) : ~0ull;
             float m_run = -INFINITY, l_run = 0.0f;
             const long long off = (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)r * p.sSlice + (long long)(it.q0 + row) * p.sPos;
@@ -328,7 +328,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 }
                 op[j] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
-            const long long loff = (long long)it.b * N * p.H * N + (long long)it.h * N + (long long)r * p.lR + (long long)(it.q0 + row) * p.lQ;
+            const long long loff = (long long)it.b * p.lB + (long long)it.h * N + (long long)r * p.lR + (long long)(it.q0 + row) * p.lQ;
             LSE[loff] = l_run > 0.0f ? m_run * kLn2 + __logf(l_run) : -INFINITY;
         }
     }
@@ -373,10 +373,10 @@ __global__ void __launch_bounds__(128) pack_mask_kernel(const unsigned char* __r
     const int lane = threadIdx.x & 31, w = blockIdx.x * 4 + (threadIdx.x >> 5);
     const int r = blockIdx.y, b = blockIdx.z, NW = p.N / 64;
     if (w >= NW) return;
-    const unsigned char* base = mask + (long long)b * p.N * p.N + (long long)r * p.mR;
+    const unsigned char* base = mask + (long long)b * p.mB + (long long)r * p.mR;
     const unsigned lo = __ballot_sync(0xffffffffu, base[(long long)(w * 64 + lane) * p.mK] != 0);
     const unsigned hi = __ballot_sync(0xffffffffu, base[(long long)(w * 64 + 32 + lane) * p.mK] != 0);
-    if (lane == 0) bits[((long long)b * p.N + r) * NW + w] = (unsigned long long)lo | ((unsigned long long)hi << 32);
+    if (lane == 0) bits[((long long)b * p.R + r) * NW + w] = (unsigned long long)lo | ((unsigned long long)hi << 32);
 }
 
 int sm_count() {
@@ -405,16 +405,18 @@ tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int 
 
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st) {
     ProfScope ps("pack_mask_kernel", st);
-    pack_mask_kernel<<<dim3((p.N / 64 + 3) / 4, p.N, p.B), 128, 0, st>>>(mask, (unsigned long long*)bits, p);
+    pack_mask_kernel<<<dim3((p.N / 64 + 3) / 4, p.R, p.B), 128, 0, st>>>(mask, (unsigned long long*)bits, p);
     return TRI_OK;
 }
 
 int sm100_sm_count() { return sm_count(); }
 
 // N <= 2048: the fused dQ + dBias stage needs one cluster rank per two 64-key tiles (<= 16 ranks)
-bool sm100_supported(const Problem& p, tri_dtype dt) { return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0 && p.N <= 2048; }
+bool sm100_supported(const Problem& p, tri_dtype dt) {
+    return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0 && p.N <= 2048 && p.R % 4 == 0 && (p.R == p.N || p.variant == TRI_STARTING);
+}
 
-size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.N * (p.N / 64) * 8, 256); }
+size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.R * (p.N / 64) * 8, 256); }
 
 size_t sm100_fwd_workspace(const Problem& p) {
     return sm100_maskbits_bytes(p) + align_up((size_t)p.B * p.H * p.N * p.N * 4, 256);  // + log2e * bias[q][k], fp32
@@ -438,12 +440,12 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
         TRI_LAUNCH_CHECK("bias_planes_kernel");
     }
     CUtensorMap tQ, tK, tV, tB;
-    if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK) ||
-        !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK) || !make_tmap_plane_f32(&tB, biasL, p.B * p.H, p.N, BQ))
+    if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ, p.R) || !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BK, p.R) ||
+        !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK, p.R) || !make_tmap_plane_f32(&tB, biasL, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
     TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));
-    const long long items = (long long)p.B * p.H * (p.N / BQ) * (p.N / NG);
+    const long long items = (long long)p.B * p.H * (p.N / BQ) * (p.R / NG);
     const int grid = (int)(items < sm_count() ? items : sm_count());
     {
         ProfScope ps("sm100_fwd_kernel", st);

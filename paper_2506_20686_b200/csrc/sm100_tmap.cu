@@ -65,18 +65,19 @@ bool cached(const TmapKey& key, CUtensorMap* out, F&& encode) {
 
 }  // namespace
 
-bool make_tmap_u(CUtensorMap* out_, const void* base, int B, int N, int H, int d, int variant, int box_pos) {
+bool make_tmap_u(CUtensorMap* out_, const void* base, int B, int N, int H, int d, int variant, int box_pos, int rows) {
+    const int R = rows < 0 ? N : rows;  // broadcast rows (starting node: the first N axis)
     TmapKey key;
     memset(&key, 0, sizeof(key));
-    key.kind = 0; key.base = base; key.a = B; key.b = N; key.c = H; key.d = d; key.e = variant; key.f = box_pos;
+    key.kind = 0; key.base = base; key.a = B; key.b = N; key.c = H; key.d = d; key.e = variant * 65536 + R; key.f = box_pos;
     return cached(key, out_, [&](CUtensorMap* out) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t es = 2;
     const cuuint64_t s_c = (cuuint64_t)d * es, s_h = (cuuint64_t)N * d * es, s_a = (cuuint64_t)H * N * d * es,
-                     s_b = (cuuint64_t)N * H * N * d * es;
+                     s_b = (cuuint64_t)R * H * N * d * es;
     // dims: (d, pos, row, h, b)
-    cuuint64_t dims[5] = {(cuuint64_t)d, (cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)H, (cuuint64_t)B};
+    cuuint64_t dims[5] = {(cuuint64_t)d, (cuuint64_t)N, (cuuint64_t)R, (cuuint64_t)H, (cuuint64_t)B};
     cuuint64_t strides[4];
     if (variant == TRI_STARTING) { strides[0] = s_c; strides[1] = s_a; } else { strides[0] = s_a; strides[1] = s_c; }
     strides[2] = s_h;

@@ -141,6 +141,67 @@ tri_status tri_attn_bwd(const void* dO, const void* Q, const void* K, const void
     return simt_bwd(p, dtype, dO, Q, K, V, G, bias, mask, O, LSE, dQ, dK, dV, dG, dBias, workspace, st);
 }
 
+// ---- decoupled row count (starting node): R broadcast rows that attend over N positions with one [B,H,N,N] bias ----
+static bool rows_ok(int B, int R, int N, int H, int d, tri_dtype dtype) {
+    if (!shape_ok(B, N, H, d) || R <= 0 || !d_ok(d) || !size_ok(B, R > N ? R : N, H, d)) return false;
+    return sm100_supported(make_problem(B, N, H, d, TRI_STARTING, R), dtype);
+}
+
+size_t tri_attn_rows_fwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype) {
+    if (!rows_ok(B, R, N, H, d, dtype)) return 0;
+    const size_t w = sm100_fwd_workspace(make_problem(B, N, H, d, TRI_STARTING, R));
+    return w < 256 ? 256 : w;
+}
+
+size_t tri_attn_rows_bwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype) {
+    if (!rows_ok(B, R, N, H, d, dtype)) return 0;
+    const size_t w = sm100_bwd_workspace(make_problem(B, N, H, d, TRI_STARTING, R));
+    return w < 256 ? 256 : w;
+}
+
+tri_status tri_attn_rows_fwd(const void* Q, const void* K, const void* V, const void* G, const void* bias,
+                             const unsigned char* mask, void* O, float* LSE, int B, int R, int N, int H, int d,
+                             tri_dtype dtype, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!shape_ok(B, N, H, d) || R <= 0 || !enums_ok(TRI_STARTING, dtype)) return TRI_ERR_INVALID_ARG;
+    if (!Q || !K || !V || !G || !bias || !O || !LSE) return TRI_ERR_INVALID_ARG;
+    if (!al16(Q) || !al16(K) || !al16(V) || !al16(G) || !al16(bias) || !al16(O) || !al16(LSE)) return TRI_ERR_INVALID_ARG;
+    if (!rows_ok(B, R, N, H, d, dtype)) return TRI_ERR_UNSUPPORTED;
+    const size_t need = tri_attn_rows_fwd_workspace_bytes(B, R, N, H, d, dtype);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TRI_ERR_WORKSPACE;
+    {
+        const size_t U = (size_t)B * R * H * N * d * 2, P = (size_t)B * H * N * N;
+        const Range r[] = {{Q, U, false}, {K, U, false}, {V, U, false}, {G, U, false}, {bias, P * 2, false},
+                           {mask, (size_t)B * R * N, false}, {O, U, true}, {LSE, (size_t)B * R * H * N * 4, true},
+                           {workspace, need, true}};
+        if (aliasing(r, 9)) return TRI_ERR_INVALID_ARG;
+    }
+    return sm100_fwd(make_problem(B, N, H, d, TRI_STARTING, R), Q, K, V, G, bias, mask, O, LSE, workspace, (cudaStream_t)cuda_stream);
+}
+
+tri_status tri_attn_rows_bwd(const void* dO, const void* Q, const void* K, const void* V, const void* G, const void* bias,
+                             const unsigned char* mask, const void* O, const float* LSE, void* dQ, void* dK, void* dV,
+                             void* dG, float* dBias, int B, int R, int N, int H, int d, tri_dtype dtype, void* workspace,
+                             size_t workspace_bytes, void* cuda_stream) {
+    if (!shape_ok(B, N, H, d) || R <= 0 || !enums_ok(TRI_STARTING, dtype)) return TRI_ERR_INVALID_ARG;
+    if (!dO || !Q || !K || !V || !G || !bias || !O || !LSE || !dQ || !dK || !dV || !dG || !dBias) return TRI_ERR_INVALID_ARG;
+    if (!al16(dO) || !al16(Q) || !al16(K) || !al16(V) || !al16(G) || !al16(bias) || !al16(O) || !al16(LSE) ||
+        !al16(dQ) || !al16(dK) || !al16(dV) || !al16(dG) || !al16(dBias))
+        return TRI_ERR_INVALID_ARG;
+    if (!rows_ok(B, R, N, H, d, dtype)) return TRI_ERR_UNSUPPORTED;
+    const size_t need = tri_attn_rows_bwd_workspace_bytes(B, R, N, H, d, dtype);
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TRI_ERR_WORKSPACE;
+    {
+        const size_t U = (size_t)B * R * H * N * d * 2, P = (size_t)B * H * N * N;
+        const Range r[] = {{dO, U, false}, {Q, U, false}, {K, U, false}, {V, U, false}, {G, U, false}, {bias, P * 2, false},
+                           {mask, (size_t)B * R * N, false}, {O, U, false}, {LSE, (size_t)B * R * H * N * 4, false},
+                           {dQ, U, true}, {dK, U, true}, {dV, U, true}, {dG, U, true}, {dBias, P * 4, true},
+                           {workspace, need, true}};
+        if (aliasing(r, 15)) return TRI_ERR_INVALID_ARG;
+    }
+    return sm100_bwd(make_problem(B, N, H, d, TRI_STARTING, R), dO, Q, K, V, G, bias, mask, O, LSE, dQ, dK, dV, dG, dBias, workspace,
+                     (cudaStream_t)cuda_stream);
+}
+
 // ---- host-buffer end-to-end step --------------------------------------------------------------
 namespace {
 struct Arena {

@@ -14,6 +14,7 @@ namespace tri {
 struct Problem {
     int B, N, H, d;
     int variant;  // tri_variant
+    int R;        // broadcast rows (= N for the square pair-tensor problem; decoupled row counts: starting node only)
     // element strides of the [B,N,H,N,d] tensors
     long long sB;      // N*H*N*d
     long long sH;      // N*d
@@ -23,14 +24,19 @@ struct Problem {
     int bQ, bK;
     // mask[b,.,.]   : element (r,k) at r*mR + k*mK
     int mR, mK;
-    // LSE / D [B,N,H,N]: element (r,q) at r*lR + q*lQ (+ b*N*H*N + h*N)
+    // LSE / D [B,R,H,N]: element (r,q) at r*lR + q*lQ (+ b*lB + h*N)
     long long lR, lQ;
+    long long lB;  // R*H*N
+    long long mB;  // mask batch stride R*N
 };
 
-inline Problem make_problem(int B, int N, int H, int d, int variant) {
+inline Problem make_problem(int B, int N, int H, int d, int variant, int R = -1) {
     Problem p;
-    p.B = B; p.N = N; p.H = H; p.d = d; p.variant = variant;
-    p.sB = (long long)N * H * N * d;
+    if (R < 0) R = N;
+    p.B = B; p.N = N; p.H = H; p.d = d; p.variant = variant; p.R = R;
+    p.sB = (long long)R * H * N * d;
+    p.lB = (long long)R * H * N;
+    p.mB = (long long)R * N;
     p.sH = (long long)N * d;
     if (variant == TRI_STARTING) {
         p.sSlice = (long long)H * N * d; p.sPos = d;

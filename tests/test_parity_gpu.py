@@ -335,3 +335,57 @@ def test_bf16_odd_batch_and_head_counts_full(tri, oracle, variant):
     """B=3, H=3 (not powers of two) on the tensor-core path, N=128: block-index decoding and per-(b,h) bias planes."""
     cfg = tri_inputs.small_config(3, 128, 3, 32, "bf16", variant, 1.0, "lengths:100,128,77", seed=333)
     full_compare(oracle, cfg)
+
+
+@pytest.mark.parametrize("R,N", [(64, 256), (192, 384), (4, 128), (100, 128), (512, 256)])
+def test_rows_decoupled_from_n_full(tri, oracle, R, N):
+    """SURVEY Sec. 8 f4 (first slice): R broadcast rows != N positions through tri_attn_rows_fwd / tri_attn_rows_bwd
+    (starting-node layout [B,R,H,N,d], mask [B,R,N], one [B,H,N,N] bias summed over the R rows in dBias).  Inputs are a
+    seeded square problem of side max(R,N) cut down to R rows and N positions (cutting keeps the values bf16-exact);
+    the mask has ragged tails, dead 64-key tiles and one fully masked row.  Every element against the oracle's general
+    starting-node routine."""
+    B, H, d, M = 2, 3, 32, max(R, N)
+    cfg = tri_inputs.small_config(B, M, H, d, "bf16", STARTING, 1.5, "none", seed=4000 + R + N)
+    sq = tri_inputs.make_inputs(cfg)
+    x = {k: np.ascontiguousarray(sq[k][:, :R, :, :N, :]) for k in ("Q", "K", "V", "G", "dO")}
+    x["bias"] = np.ascontiguousarray(sq["bias"][:, :, :N, :N])
+    rng = np.random.default_rng(R * 7 + N)
+    m = np.ones((B, R, N), np.uint8)
+    for b in range(B):
+        for r in range(R):
+            kind = (r + b) % 4
+            if kind == 1:
+                m[b, r, N - int(rng.integers(1, N // 2)):] = 0
+            elif kind == 2:
+                m[b, r, :64 * int(rng.integers(1, N // 64))] = 0
+            elif kind == 3:
+                m[b, r] = rng.random(N) < 0.8
+    m[0, R // 2, :] = 0
+    x["mask"] = m
+    g = pu.gpu_inputs(x, "bf16")
+    O, LSE = tri.tri_attn_rows_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"])
+    outs = tri.tri_attn_rows_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], O, LSE)
+    import torch
+
+    torch.cuda.synchronize()
+    got = {k: v.float().cpu().numpy().astype(np.float64) for k, v in zip(pu.OUT_NAMES, (O, LSE) + tuple(outs))}
+    rO, rLSE = oracle.fwd_start_general(x["Q"], x["K"], x["V"], x["G"], x["bias"], x["mask"])
+    ref = dict(zip(pu.OUT_NAMES, (rO, rLSE) + tuple(
+        oracle.bwd_start_general(x["dO"], x["Q"], x["K"], x["V"], x["G"], x["bias"], x["mask"]))))
+    errs = pu.assert_close(got, ref, pu.TOL["bf16"], what=f"rows R={R} N={N}")
+    print("rows", R, N, {k: float(f"{v:.3g}") for k, v in errs.items()})
+    assert np.isneginf(got["LSE"][0, R // 2]).all()
+
+
+def test_rows_entry_points_reject_what_the_tensor_core_path_cannot_run(tri):
+    import torch
+
+    B, R, N, H = 1, 6, 128, 2  # R % 4 != 0
+    q = torch.zeros((B, R, H, N, 32), dtype=torch.bfloat16, device="cuda")
+    bias = torch.zeros((B, H, N, N), dtype=torch.bfloat16, device="cuda")
+    assert tri.rows_fwd_workspace_bytes(B, R, N, H, 32, tri.BF16) == 0
+    with pytest.raises(tri.TriAttnError, match="UNSUPPORTED"):
+        tri.tri_attn_rows_fwd(q, q.clone(), q.clone(), q.clone(), bias)
+    assert tri.rows_fwd_workspace_bytes(B, 8, N, H, 32, tri.F32) == 0
+    assert tri.rows_fwd_workspace_bytes(B, 8, N, H, 32, tri.BF16) > 0
+    assert tri.rows_bwd_workspace_bytes(B, 8, 192, H, 32, tri.BF16) == 0
