@@ -51,6 +51,11 @@
  *     caller it is still one unit of work on that stream).  Each element is solved as a B = 1
  *     problem: identical to tri_attn_fwd/bwd on that element alone, which for dBias can differ in the
  *     last bits from a B > 1 call (the row split of the deterministic reduction depends on B).
+ *     On the tensor-core path of the starting-node variant the broadcast rows of an element are
+ *     independent too, so an element is further cut into about eight row chunks (>= 4 MB per tensor,
+ *     each run as a tri_attn_rows_* problem): O, LSE, dQ, dK, dV, dG stay bitwise those of
+ *     tri_attn_fwd/bwd, dBias is accumulated chunk after chunk in row order (same fp32 sum, another
+ *     grouping; still bitwise reproducible run to run).
  *   - Errors: a tri_status is returned, nothing is thrown or aborted across the ABI.  Argument
  *     errors are detected before any launch.  Launch failures map to TRI_ERR_CUDA.
  *   - Supported: d in {16, 32, 64}, any N >= 1, dtype f32 or bf16.  bf16 with d == 32 and

@@ -53,15 +53,16 @@ __global__ void __launch_bounds__(256) sm100_bwd_pre_kernel(long long rows, cons
 
 // level 2 of the dBias reduction (only when the row axis was split): dBias[bh][q*bQ + k*bK] = sum over planes, in
 // ascending order, of plane[g][bh][q][k]; the ending-node variant wants the transpose (bQ = 1), via a 32x32 smem tile.
+// accumulate != 0 (starting node only): the sum starts from the value dBias already holds (row-chunked callers).
 __global__ void __launch_bounds__(256) sm100_dbias_reduce_kernel(const float* __restrict__ planes, float* __restrict__ dBias,
-                                                                 int BH, int N, int G, int transpose) {
+                                                                 int BH, int N, int G, int transpose, int accumulate) {
     __shared__ float tile[32][33];
     const int bh = blockIdx.z, q0 = blockIdx.y * 32, k0 = blockIdx.x * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const long long pstride = (long long)BH * N * N;
     for (int j = ty; j < 32; j += 8) {
         const long long o = (long long)bh * N * N + (long long)(q0 + j) * N + k0 + tx;
-        float acc = planes[o];
+        float acc = accumulate ? dBias[o] + planes[o] : planes[o];
         for (int g = 1; g < G; ++g) acc += planes[o + g * pstride];
         if (transpose) tile[j][tx] = acc; else dBias[o] = acc;
     }
@@ -126,7 +127,8 @@ size_t sm100_bwd_workspace(const Problem& p) { return bwd_ws_layout(p).total; }
 
 tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void* K, const void* V, const void* G,
                      const void* bias, const unsigned char* mask, const void* O, const float* LSE, void* dQ, void* dK,
-                     void* dV, void* dG, float* dBias, void* ws, cudaStream_t st) {
+                     void* dV, void* dG, float* dBias, void* ws, cudaStream_t st, bool accumulate_dbias) {
+    if (accumulate_dbias && p.variant != TRI_STARTING) return TRI_ERR_UNSUPPORTED;
     const BwdWs w = bwd_ws_layout(p);
     float* Dws = (float*)((char*)ws + w.d_off);
     void* dA = (char*)ws + w.da_off;
@@ -180,7 +182,8 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
         TRI_CUDA_CHECK(cudaEventRecord(side->fork, st));
         TRI_CUDA_CHECK(cudaStreamWaitEvent(side->stream, side->fork, 0));
     }
-    if ((s = sm100_dqdb_launch(p, C2, Gs, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dBias, planes, st)) != TRI_OK) return s;
+    if ((s = sm100_dqdb_launch(p, C2, Gs, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, accumulate_dbias ? planes : dBias, planes, st)) != TRI_OK)
+        return s;
     if (itemsA > 0) {
         if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, NL, ND, dK, dV, 0, itemsA, spare, "sm100_dkdv_kernel(side)",
                                     side->stream)) != TRI_OK)
@@ -191,11 +194,11 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
         TRI_OK)
         return s;
     if (itemsA > 0) TRI_CUDA_CHECK(cudaStreamWaitEvent(st, side->join, 0));
-    if (Gs > 1) {
+    if (Gs > 1 || accumulate_dbias) {
         {
             ProfScope ps("sm100_dbias_reduce_kernel", st);
             sm100_dbias_reduce_kernel<<<dim3(p.N / 32, p.N / 32, p.B * p.H), 256, 0, st>>>(
-                planes, dBias, p.B * p.H, p.N, Gs, p.variant == TRI_ENDING ? 1 : 0);
+                planes, dBias, p.B * p.H, p.N, Gs, p.variant == TRI_ENDING ? 1 : 0, accumulate_dbias ? 1 : 0);
         }
         TRI_LAUNCH_CHECK("sm100_dbias_reduce_kernel");
     }

@@ -28,7 +28,7 @@ EncodeTiledFn encode_fn() {
 }
 
 // Descriptor cache: a CUtensorMap is a pure function of (kind, base pointer, shape, variant, box), and a training loop
-// calls with the same buffers every step, so the driver's encode runs once per distinct key (bounded: flushed at 512 keys).
+// calls with the same buffers every step, so the driver's encode runs once per distinct key (bounded: flushed at 4096 keys).
 struct TmapKey {
     int kind;
     const void* base;
@@ -58,7 +58,7 @@ bool cached(const TmapKey& key, CUtensorMap* out, F&& encode) {
     }
     if (!encode(out)) return false;
     std::lock_guard<std::mutex> lock(g_tmap_mu);
-    if (g_tmap_cache.size() >= 512) g_tmap_cache.clear();
+    if (g_tmap_cache.size() >= 4096) g_tmap_cache.clear();
     g_tmap_cache.emplace(key, *out);
     return true;
 }

@@ -263,11 +263,13 @@ struct HostPipe {
 HostPipe g_pipes[64];  // one per device ordinal
 }  // namespace
 
-// Batch elements are independent problems (every tensor has B as its outermost axis), so the step runs as a
-// three-stage pipeline over b: H2D of element b+1 (copy stream) || forward + backward of element b (the caller's
-// stream) || D2H of element b-1 (second copy stream).  Inside an element the dO copy overlaps the forward and the
-// O / LSE read-back overlaps the backward.  Everything is forked from and joined back into `cuda_stream` with events,
-// so the call still behaves as one unit of work enqueued on that stream, and the host is never blocked.
+// Batch elements are independent problems (every tensor has B as its outermost axis), and on the tensor-core path of
+// the starting-node variant so are the broadcast rows of one element (all tensors but bias / dBias have the row as
+// their second axis; dBias is accumulated chunk after chunk, in row order).  The step therefore runs as a three-stage
+// pipeline over chunks: H2D of chunk c+1 (copy stream) || forward + backward of chunk c (the caller's stream) || D2H
+// of chunk c-1 (second copy stream).  Inside a chunk the dO copy overlaps the forward and the O / LSE read-back overlaps
+// the backward.  Everything is forked from and joined back into `cuda_stream` with events, so the call still behaves
+// as one unit of work enqueued on that stream, and the host is never blocked.
 tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, const void* hG, const void* hbias,
                               const unsigned char* hmask, const void* hdO, void* hO, float* hLSE, void* hdQ,
                               void* hdK, void* hdV, void* hdG, float* hdBias, int B, int N, int H, int d,
@@ -289,14 +291,22 @@ tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, co
     cudaStream_t sin = g_pipe.in, sout = g_pipe.out;
     char* base = (char*)arena;
     const size_t es = dtype == TRI_F32 ? 4 : 2;
-    // pipeline chunk = one batch element when its slices keep the 16-byte pointer alignment, else the whole batch
-    const bool split = B > 1 && ((size_t)H * N * N * es) % 16 == 0 && ((size_t)N * H * N * 4) % 16 == 0;
-    const int cb = split ? 1 : B, nchunk = B / cb;
-    // per-chunk sizes (bytes)
-    const size_t u = (size_t)cb * N * H * N * d * es, pb = (size_t)cb * H * N * N * es, mb = (size_t)cb * N * N,
-                 lb = (size_t)cb * N * H * N * 4, gb = (size_t)cb * H * N * N * 4;
+    // Pipeline chunk.  Row chunks (about eight per element, at least 4 MB per tensor) when the tensor-core kernels can run
+    // a [1, rc, H, N, d] problem; else one batch element when its slices keep the 16-byte pointer alignment; else all.
+    int rc = N, cb = B;
+    if (variant == TRI_STARTING && sm100_supported(make_problem(1, N, H, d, variant), dtype)) {
+        rc = ((N + 7) / 8 + 3) / 4 * 4;
+        while (rc < N && (size_t)rc * H * N * d * es < ((size_t)4 << 20)) rc *= 2;
+        if (rc > N) rc = N;
+        cb = 1;
+    } else if (B > 1 && ((size_t)H * N * N * es) % 16 == 0 && ((size_t)N * H * N * 4) % 16 == 0) {
+        cb = 1;
+    }
+    const bool by_rows = rc < N;
+    // per-row and per-element sizes (bytes)
+    const size_t u_row = (size_t)H * N * d * es, l_row = (size_t)H * N * 4, m_row = (size_t)N;
+    const size_t pb = (size_t)H * N * N * es, gb = (size_t)H * N * N * 4;
     // arena regions: 0-3 Q K V G | 4 dO | 5 O | 6-9 dQ dK dV dG | 10 bias | 11 mask | 12 LSE | 13 dBias | 14 workspace
-    auto U_ = [&](int r, int b) { return (void*)(base + a.off[r] + (size_t)b * u); };
     size_t ne = 0;
     cudaEvent_t e0 = g_pipe.event(ne++);
     if (!e0) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: event creation");
@@ -308,43 +318,60 @@ tri_status tri_attn_step_host(const void* hQ, const void* hK, const void* hV, co
     void* hout[4] = {hdQ, hdK, hdV, hdG};
     const size_t wf = tri_attn_fwd_workspace_bytes(cb, N, H, d, variant, dtype), wb = tri_attn_bwd_workspace_bytes(cb, N, H, d, variant, dtype);
     void* ws = base + a.off[14];
-    for (int b = 0; b < nchunk; ++b) {
-        cudaEvent_t e_inA = g_pipe.event(ne++), e_inB = g_pipe.event(ne++), e_f = g_pipe.event(ne++), e_b = g_pipe.event(ne++);
-        if (!e_inA || !e_inB || !e_f || !e_b) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: event creation");
-        // ---- H2D of element b (copy stream): forward inputs, then dO
-        for (int i = 0; i < 4; ++i)
-            TRI_CUDA_CHECK(cudaMemcpyAsync(U_(i, b), (const char*)hin[i] + (size_t)b * u, u, cudaMemcpyHostToDevice, sin));
-        TRI_CUDA_CHECK(cudaMemcpyAsync(base + a.off[10] + (size_t)b * pb, (const char*)hbias + (size_t)b * pb, pb, cudaMemcpyHostToDevice, sin));
-        unsigned char* dmask = nullptr;
-        if (hmask) {
-            dmask = (unsigned char*)(base + a.off[11] + (size_t)b * mb);
-            TRI_CUDA_CHECK(cudaMemcpyAsync(dmask, hmask + (size_t)b * mb, mb, cudaMemcpyHostToDevice, sin));
+    for (int b = 0; b < B; b += cb) {
+        for (int r0 = 0; r0 < N; r0 += rc) {
+            const int nr = N - r0 < rc ? N - r0 : rc;
+            const size_t row = (size_t)b * N + r0;                                 // first global row of the chunk
+            const size_t uo = row * u_row, u = (size_t)cb * nr * u_row;            // offset / size in a [B,N,H,N,d] tensor
+            const size_t lo = row * l_row, lb = (size_t)cb * nr * l_row;           // LSE
+            const size_t mo = row * m_row, mb = (size_t)cb * nr * m_row;           // mask
+            const bool first = r0 == 0, last = r0 + nr == N;
+            auto U_ = [&](int r) { return (void*)(base + a.off[r] + uo); };
+            cudaEvent_t e_inA = g_pipe.event(ne++), e_inB = g_pipe.event(ne++), e_f = g_pipe.event(ne++), e_b = g_pipe.event(ne++);
+            if (!e_inA || !e_inB || !e_f || !e_b) return cuda_fail(cudaGetLastError(), "tri_attn_step_host: event creation");
+            // ---- H2D of the chunk (copy stream): forward inputs, then dO
+            for (int i = 0; i < 4; ++i)
+                TRI_CUDA_CHECK(cudaMemcpyAsync(U_(i), (const char*)hin[i] + uo, u, cudaMemcpyHostToDevice, sin));
+            void* dbias_in = base + a.off[10] + (size_t)b * pb;
+            if (first) TRI_CUDA_CHECK(cudaMemcpyAsync(dbias_in, (const char*)hbias + (size_t)b * pb, (size_t)cb * pb, cudaMemcpyHostToDevice, sin));
+            unsigned char* dmask = nullptr;
+            if (hmask) {
+                dmask = (unsigned char*)(base + a.off[11] + mo);
+                TRI_CUDA_CHECK(cudaMemcpyAsync(dmask, hmask + mo, mb, cudaMemcpyHostToDevice, sin));
+            }
+            TRI_CUDA_CHECK(cudaEventRecord(e_inA, sin));
+            TRI_CUDA_CHECK(cudaMemcpyAsync(U_(4), (const char*)hdO + uo, u, cudaMemcpyHostToDevice, sin));
+            TRI_CUDA_CHECK(cudaEventRecord(e_inB, sin));
+            // ---- compute of the chunk (caller's stream)
+            float* dLSE = (float*)(base + a.off[12] + lo);
+            float* gBias = (float*)(base + a.off[13] + (size_t)b * gb);
+            TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e_inA, 0));
+            tri_status s;
+            if (by_rows)
+                s = sm100_fwd(make_problem(1, N, H, d, variant, nr), U_(0), U_(1), U_(2), U_(3), dbias_in, dmask, U_(5), dLSE, ws, st);
+            else
+                s = tri_attn_fwd(U_(0), U_(1), U_(2), U_(3), dbias_in, dmask, U_(5), dLSE, cb, N, H, d, variant, dtype, ws, wf, st);
+            if (s != TRI_OK) return s;
+            TRI_CUDA_CHECK(cudaEventRecord(e_f, st));
+            TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e_inB, 0));
+            if (by_rows)
+                s = sm100_bwd(make_problem(1, N, H, d, variant, nr), U_(4), U_(0), U_(1), U_(2), U_(3), dbias_in, dmask, U_(5), dLSE, U_(6),
+                              U_(7), U_(8), U_(9), gBias, ws, st, /*accumulate_dbias=*/!first);
+            else
+                s = tri_attn_bwd(U_(4), U_(0), U_(1), U_(2), U_(3), dbias_in, dmask, U_(5), dLSE, U_(6), U_(7), U_(8), U_(9), gBias, cb, N, H,
+                                 d, variant, dtype, ws, wb, st);
+            if (s != TRI_OK) return s;
+            TRI_CUDA_CHECK(cudaEventRecord(e_b, st));
+            // ---- D2H of the chunk (second copy stream): O, LSE while the backward runs, gradients after it
+            TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e_f, 0));
+            TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hO + uo, U_(5), u, cudaMemcpyDeviceToHost, sout));
+            TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hLSE + lo, dLSE, lb, cudaMemcpyDeviceToHost, sout));
+            TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e_b, 0));
+            for (int i = 0; i < 4; ++i)
+                TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hout[i] + uo, U_(6 + i), u, cudaMemcpyDeviceToHost, sout));
+            if (last)
+                TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hdBias + (size_t)b * gb, gBias, (size_t)cb * gb, cudaMemcpyDeviceToHost, sout));
         }
-        TRI_CUDA_CHECK(cudaEventRecord(e_inA, sin));
-        TRI_CUDA_CHECK(cudaMemcpyAsync(U_(4, b), (const char*)hdO + (size_t)b * u, u, cudaMemcpyHostToDevice, sin));
-        TRI_CUDA_CHECK(cudaEventRecord(e_inB, sin));
-        // ---- compute of element b (caller's stream)
-        float* dLSE = (float*)(base + a.off[12] + (size_t)b * lb);
-        float* gBias = (float*)(base + a.off[13] + (size_t)b * gb);
-        void* dbias_in = base + a.off[10] + (size_t)b * pb;
-        TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e_inA, 0));
-        tri_status s = tri_attn_fwd(U_(0, b), U_(1, b), U_(2, b), U_(3, b), dbias_in, dmask, U_(5, b), dLSE, cb, N, H, d, variant, dtype,
-                                    ws, wf, st);
-        if (s != TRI_OK) return s;
-        TRI_CUDA_CHECK(cudaEventRecord(e_f, st));
-        TRI_CUDA_CHECK(cudaStreamWaitEvent(st, e_inB, 0));
-        s = tri_attn_bwd(U_(4, b), U_(0, b), U_(1, b), U_(2, b), U_(3, b), dbias_in, dmask, U_(5, b), dLSE, U_(6, b), U_(7, b), U_(8, b),
-                         U_(9, b), gBias, cb, N, H, d, variant, dtype, ws, wb, st);
-        if (s != TRI_OK) return s;
-        TRI_CUDA_CHECK(cudaEventRecord(e_b, st));
-        // ---- D2H of element b (second copy stream): O, LSE while the backward runs, gradients after it
-        TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e_f, 0));
-        TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hO + (size_t)b * u, U_(5, b), u, cudaMemcpyDeviceToHost, sout));
-        TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hLSE + (size_t)b * lb, dLSE, lb, cudaMemcpyDeviceToHost, sout));
-        TRI_CUDA_CHECK(cudaStreamWaitEvent(sout, e_b, 0));
-        for (int i = 0; i < 4; ++i)
-            TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hout[i] + (size_t)b * u, U_(6 + i, b), u, cudaMemcpyDeviceToHost, sout));
-        TRI_CUDA_CHECK(cudaMemcpyAsync((char*)hdBias + (size_t)b * gb, gBias, gb, cudaMemcpyDeviceToHost, sout));
     }
     // join: later work on the caller's stream waits for the last read-back (and for the copy-in stream, trivially done)
     cudaEvent_t e1 = g_pipe.event(ne++), e2 = g_pipe.event(ne++);

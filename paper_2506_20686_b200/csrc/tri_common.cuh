@@ -121,6 +121,6 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
 tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void* K, const void* V,
                      const void* G, const void* bias, const unsigned char* mask, const void* O,
                      const float* LSE, void* dQ, void* dK, void* dV, void* dG, float* dBias,
-                     void* ws, cudaStream_t st);
+                     void* ws, cudaStream_t st, bool accumulate_dbias = false);  // true: dBias += (starting node only)
 
 }  // namespace tri

@@ -284,6 +284,32 @@ def test_step_host_end_to_end_matches_device_path(tri):
         assert torch.equal(hout[k].view(torch.uint8), dev[k].cpu().view(torch.uint8)), k
 
 
+def test_step_host_row_chunked_pipeline_matches_device_path(tri):
+    """B = 2, N = 384, starting node, bf16: tri_attn_step_host cuts every element into eight 48-row chunks (copy in ||
+    compute || copy out) and accumulates dBias chunk after chunk.  Rows are independent, so every output but dBias is
+    bitwise what the device path gives; dBias is the same fp32 sum in another grouping (<= 1e-5 of its max)."""
+    import torch
+
+    cfg = tri_inputs.small_config(2, 384, 4, 32, "bf16", STARTING, 1.0, "lengths:300,384", seed=77)
+    x = tri_inputs.make_inputs(cfg)
+    _, dev = pu.run_gpu(x, cfg.dtype, cfg.variant)
+    hin = {k: pu.to_torch(x[k], cfg.dtype, "cpu").pin_memory() for k in ("Q", "K", "V", "G", "bias", "dO")}
+    hin["mask"] = torch.from_numpy(x["mask"]).pin_memory()
+    B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
+    hout = {k: torch.full_like(hin["Q"], float("nan")).pin_memory() for k in ("O", "dQ", "dK", "dV", "dG")}
+    hout["LSE"] = torch.full((B, N, H, N), float("nan"), dtype=torch.float32).pin_memory()
+    hout["dBias"] = torch.full((B, H, N, N), float("nan"), dtype=torch.float32).pin_memory()
+    arena = torch.empty(tri.step_host_arena_bytes(B, N, H, d, cfg.variant, tri.BF16), dtype=torch.uint8, device="cuda")
+    for _ in range(2):  # the second call re-uses the arena (dBias must be overwritten, not accumulated into)
+        tri.tri_attn_step_host(hin, hout, cfg.variant, arena)
+        torch.cuda.synchronize()
+        for k in pu.OUT_NAMES:
+            if k != "dBias":
+                assert torch.equal(hout[k].view(torch.uint8), dev[k].cpu().view(torch.uint8)), k
+        ref = dev["dBias"].cpu().double()
+        assert float((hout["dBias"].double() - ref).abs().max() / ref.abs().max()) <= 1e-5
+
+
 def test_step_host_pipelines_batch_elements(tri, oracle):
     """B = 3: tri_attn_step_host overlaps the copies and the compute of different batch elements; each element must be
     bitwise what tri_attn_fwd / tri_attn_bwd give for that element alone, and the whole must match the oracle."""
