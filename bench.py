@@ -448,6 +448,64 @@ def run_ours(args, cfg):
     print(json.dumps(line))
 
 
+def run_evosp(args, cfg):
+    """--sp: EvoSP-3D strong scaling of ONE batch: the broadcast rows are
+    sharded over the ranks, the step is bias all-gather -> rows forward -> rows backward -> dBias reduce-scatter
+    (paper_2506_20686_b200/evosp.py).  Not the driver's default line (that one is weak scaling without collectives)."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_2506_20686_b200 as tri
+    from paper_2506_20686_b200 import evosp
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU path)")
+    if cfg.variant != tri_inputs.STARTING:
+        raise SystemExit("bench.py --sp: starting-node workloads only (rotate() the operands for the ending node)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if not dist.is_initialized():
+        if world > 1:
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29517", rank=0, world_size=1, device_id=dev)
+    tri.load()
+    r0, n = evosp.shard_rows(cfg.N, world, rank)
+    x = tri_inputs.make_inputs(cfg)  # the same batch on every rank; each keeps its rows
+    tdt = torch.bfloat16
+    g = {k: torch.from_numpy(x[k][:, r0:r0 + n].copy()).to(tdt).to(dev) for k in ("Q", "K", "V", "G", "dO")}
+    bias_shard = torch.from_numpy(x["bias"][:, :, r0:r0 + n].copy()).to(tdt).to(dev)
+    mask = None if x["mask"] is None else torch.from_numpy(x["mask"][:, r0:r0 + n].copy()).to(dev)
+    op = evosp.RowShardedTriAttention()
+
+    def step():
+        op.forward(g["Q"], g["K"], g["V"], g["G"], bias_shard, mask)
+        op.backward(g["dO"])
+
+    for _ in range(args.warmup):
+        step()
+    dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    dist.barrier()
+    torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1) / args.steps, dev, world)
+    if rank == 0:
+        print(json.dumps({
+            "metric": "triangle-attn fwd+bwd TFLOP/s", "value": model_flop(cfg) / (ms * 1e-3) / 1e12, "unit": "TFLOP/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "parallelism": f"sp{world}: {n} of {cfg.N} rows per rank, "
+                       "bias all-gather + dBias reduce-scatter inside the step"}}))
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -455,11 +513,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=sorted(tri_inputs.CONFIGS))
+    ap.add_argument("--sp", action="store_true", help="EvoSP-3D row sharding of one batch (strong scaling)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = tri_inputs.CONFIGS[args.workload]
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.sp:
+        run_evosp(args, cfg)
     else:
         run_ours(args, cfg)
 

@@ -415,3 +415,45 @@ def test_rows_entry_points_reject_what_the_tensor_core_path_cannot_run(tri):
     assert tri.rows_fwd_workspace_bytes(B, 8, N, H, 32, tri.F32) == 0
     assert tri.rows_fwd_workspace_bytes(B, 8, N, H, 32, tri.BF16) > 0
     assert tri.rows_bwd_workspace_bytes(B, 8, 192, H, 32, tri.BF16) == 0
+
+
+def test_evosp_row_shards_reproduce_the_unsharded_kernels(tri):
+    """SURVEY Sec. 8(e) / f2 on one GPU: (1) RowShardedTriAttention on a single-rank NCCL group (all-gather and
+    reduce-scatter degenerate to copies) equals tri_attn_fwd / tri_attn_bwd; (2) the P = 2 and P = 3 row shards of
+    evosp.shard_rows, run one after another through the rows entry points, give bitwise the unsharded O, LSE, dQ, dK,
+    dV, dG, and partial dBias planes whose sum is the unsharded dBias up to fp32 regrouping."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2506_20686_b200 import evosp
+
+    cfg = tri_inputs.small_config(1, 384, 2, 32, "bf16", STARTING, 1.0, "tail:40", seed=31)
+    x = tri_inputs.make_inputs(cfg)
+    _, full = pu.run_gpu(x, "bf16", STARTING)
+    g = pu.gpu_inputs(x, "bf16")
+    names = ("O", "LSE", "dQ", "dK", "dV", "dG")
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29519", rank=0, world_size=1,
+                                device_id=torch.device("cuda", 0))
+    try:
+        op = evosp.RowShardedTriAttention()
+        O, LSE = op.forward(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"])
+        outs = (O, LSE) + tuple(op.backward(g["dO"]))
+        torch.cuda.synchronize()
+        for k, v in zip(pu.OUT_NAMES, outs):
+            assert torch.equal(v, full[k]), k
+    finally:
+        dist.destroy_process_group()
+    for P in (2, 3):
+        dsum = torch.zeros_like(full["dBias"], dtype=torch.float64)
+        for rank in range(P):
+            r0, n = evosp.shard_rows(cfg.N, P, rank)
+            loc = {k: g[k][:, r0:r0 + n].contiguous() for k in ("Q", "K", "V", "G", "dO", "mask")}
+            O, LSE = tri.tri_attn_rows_fwd(loc["Q"], loc["K"], loc["V"], loc["G"], g["bias"], loc["mask"])
+            outs = (O, LSE) + tuple(tri.tri_attn_rows_bwd(loc["dO"], loc["Q"], loc["K"], loc["V"], loc["G"], g["bias"],
+                                                          loc["mask"], O, LSE))
+            for k, v in zip(names, outs[:6]):
+                assert torch.equal(v, full[k][:, r0:r0 + n]), (P, rank, k)
+            dsum += outs[6].double()
+        ref = full["dBias"].double()
+        assert float((dsum - ref).abs().max() / ref.abs().max()) <= 1e-5
