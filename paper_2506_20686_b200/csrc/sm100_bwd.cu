@@ -61,6 +61,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_reduce_kernel(const float* __
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const long long pstride = (long long)BH * N * N;
     for (int j = ty; j < 32; j += 8) {
+        if (q0 + j >= N || k0 + tx >= N) continue;
         const long long o = (long long)bh * N * N + (long long)(q0 + j) * N + k0 + tx;
         float acc = accumulate ? dBias[o] + planes[o] : planes[o];
         for (int g = 1; g < G; ++g) acc += planes[o + g * pstride];
@@ -68,7 +69,8 @@ __global__ void __launch_bounds__(256) sm100_dbias_reduce_kernel(const float* __
     }
     if (transpose) {
         __syncthreads();
-        for (int j = ty; j < 32; j += 8) dBias[(long long)bh * N * N + (long long)(k0 + j) * N + q0 + tx] = tile[tx][j];
+        for (int j = ty; j < 32; j += 8)
+            if (k0 + j < N && q0 + tx < N) dBias[(long long)bh * N * N + (long long)(k0 + j) * N + q0 + tx] = tile[tx][j];
     }
 }
 
@@ -146,7 +148,7 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     const void* bias_kq = p.variant == TRI_STARTING ? biasT : bias;  // [k][q]
 
     unsigned long long* maskbits = nullptr;
-    if (mask) {
+    if (sm100_needs_maskbits(p, mask)) {
         maskbits = (unsigned long long*)((char*)ws + w.mask_off);
         if ((s = sm100_pack_mask(p, mask, maskbits, st)) != TRI_OK) return s;
         TRI_LAUNCH_CHECK("pack_mask_kernel");
@@ -197,7 +199,7 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     if (Gs > 1 || accumulate_dbias) {
         {
             ProfScope ps("sm100_dbias_reduce_kernel", st);
-            sm100_dbias_reduce_kernel<<<dim3(p.N / 32, p.N / 32, p.B * p.H), 256, 0, st>>>(
+            sm100_dbias_reduce_kernel<<<dim3((p.N + 31) / 32, (p.N + 31) / 32, p.B * p.H), 256, 0, st>>>(
                 planes, dBias, p.B * p.H, p.N, Gs, p.variant == TRI_ENDING ? 1 : 0, accumulate_dbias ? 1 : 0);
         }
         TRI_LAUNCH_CHECK("sm100_dbias_reduce_kernel");

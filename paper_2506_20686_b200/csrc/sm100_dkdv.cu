@@ -58,7 +58,7 @@ struct ItemK { int b, h, k0, r0; };
 // then from L2) instead of streaming the whole pair tensor once per key block
 __device__ __forceinline__ ItemK decode_itemk(int item, int N, int H, int NT3) {
     ItemK it;
-    const int NKB = N / BKEY;
+    const int NKB = (N + BKEY - 1) / BKEY;
     it.k0 = (item % NKB) * BKEY;
     int t = item / NKB;
     it.r0 = (t % NT3) * NGK;
@@ -121,9 +121,11 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int N = p.N, NW = N / 64;
+    const int N = p.N, NW = (N + 63) / 64;
     const int NT3 = (p.R + NGK - 1) / NGK;  // row triples (the last one may be partial)
-    const int NS = N / BQS;               // ring stages per row
+    const int NS = (N + BQS - 1) / BQS;   // ring stages per row (the last one may be partial: TMA zero-fills Q / dA / bias^T,
+                                          // NL is -inf there, so P^T = dS^T = 0 for queries >= N;
+                                          // NL / ND rows are padded to NS * BQS by lse_prep_kernel)
     const int n_items = (total_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
 
     if (tid == 0) {
@@ -171,7 +173,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                         for (int g = 0; g < nr; ++g) {
                             tma_load_5d(st + g * 2 * QS_BYTES, &tmQ, full + s, 0, sq * BQS, it.r0 + g, it.h, it.b);
                             tma_load_5d(st + g * 2 * QS_BYTES + QS_BYTES, &tmA, full + s, 0, sq * BQS, it.r0 + g, it.h, it.b);
-                            const long long o = (((long long)it.b * p.R + it.r0 + g) * p.H + it.h) * N + sq * BQS;
+                            const long long o = ((((long long)it.b * p.R + it.r0 + g) * p.H + it.h) * NS + sq) * BQS;  // row pitch NS * BQS
                             float* ld = (float*)(st + NGK * 2 * QS_BYTES + BIAS_BYTES) + g * 2 * BQS;
                             bulk_load(ld, NL + o, BQS * 4, full + s);
                             bulk_load(ld + BQS, ND + o, BQS * 4, full + s);
@@ -291,8 +293,8 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
             const int r = it.r0 + g;
             const bool active = r < p.R;
-            bool keep = true;
-            if (active && maskbits)
+            bool keep = it.k0 + row < N;  // keys beyond N of the last (partial) key block are TMA zero-fill
+            if (active && keep && maskbits)
                 keep = (ldg_u64(maskbits + ((long long)it.b * p.R + r) * NW + (it.k0 + row) / 64) >> ((it.k0 + row) & 63)) & 1ull;
             const bool allkeep = __all_sync(0xffffffffu, keep);
             for (int sq = 0; sq < NS; ++sq, ++n) {
@@ -360,6 +362,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                 const long long off = (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)r * p.sSlice + (long long)(it.k0 + row) * p.sPos;
                 uint4* pv = (uint4*)(dV + off);
                 uint4* pk = (uint4*)(dK + off);
+                if (it.k0 + row >= N) continue;  // keys beyond N of the last (partial) key block: nothing to store
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     uint32_t a[4], c[4];
@@ -380,14 +383,20 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
 }
 
 // -LSE*log2e (-inf for fully masked queries) and -D as [B][row][H][query] in the variant's (row, query) sense, so a unit's
-// 32 queries are contiguous for both variants
+// 32 queries are contiguous for both variants.  The query axis is padded to whole 64-query stages with NL = -inf, ND = 0.
 __global__ void __launch_bounds__(256) lse_prep_kernel(const float* __restrict__ LSE, const float* __restrict__ Dws,
                                                        float* __restrict__ NL, float* __restrict__ ND, Problem p) {
-    const long long total = (long long)p.B * p.R * p.H * p.N;
+    const int NPQ = (p.N + BQS - 1) / BQS * BQS;
+    const long long total = (long long)p.B * p.R * p.H * NPQ;
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= total) return;
-    const int q = (int)(i % p.N);
-    long long t = i / p.N;
+    const int q = (int)(i % NPQ);
+    long long t = i / NPQ;
+    if (q >= p.N) {
+        NL[i] = -INFINITY;
+        ND[i] = 0.0f;
+        return;
+    }
     const int h = (int)(t % p.H);
     t /= p.H;
     const int r = (int)(t % p.R);
@@ -400,12 +409,12 @@ __global__ void __launch_bounds__(256) lse_prep_kernel(const float* __restrict__
 
 }  // namespace
 
-size_t sm100_dkdv2_aux_bytes(const Problem& p) { return align_up((size_t)p.B * p.R * p.H * p.N * 4, 256); }
+size_t sm100_dkdv2_aux_bytes(const Problem& p) { return align_up((size_t)p.B * p.R * p.H * ((p.N + BQS - 1) / BQS * BQS) * 4, 256); }
 
-long long sm100_dkdv2_items(const Problem& p) { return (long long)p.B * p.H * (p.N / BKEY) * ((p.R + NGK - 1) / NGK); }
+long long sm100_dkdv2_items(const Problem& p) { return (long long)p.B * p.H * ((p.N + BKEY - 1) / BKEY) * ((p.R + NGK - 1) / NGK); }
 
 tri_status sm100_lse_prep(const Problem& p, const float* LSE, const float* Dws, float* NL, float* ND, cudaStream_t st) {
-    const long long total = (long long)p.B * p.R * p.H * p.N;
+    const long long total = (long long)p.B * p.R * p.H * ((p.N + BQS - 1) / BQS * BQS);
     {
         ProfScope ps("lse_prep_kernel", st);
         lse_prep_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(LSE, Dws, NL, ND, p);

@@ -128,7 +128,7 @@ struct Item2 { int b, h, q0, rb; };
 // query block fastest: clusters that run concurrently work on the same rows (K_r, V_r shared through L2)
 __device__ __forceinline__ Item2 decode_item2(int item, int N, int H, int G, int NR) {
     Item2 it;
-    const int NQB = N / BQ;
+    const int NQB = (N + BQ - 1) / BQ;
     it.q0 = (item % NQB) * BQ;
     int t = item / NQB;
     it.rb = (t % G) * NR;
@@ -169,7 +169,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int N = p.N, NW = N / BK;
+    const int N = p.N, NW = (N + BK - 1) / BK;  // the last tile / query block may be partial (TMA zero-fill + mask bits)
     const int C = (int)cluster_nctarank(), c = (int)cluster_ctarank();
     // key tiles of this rank: the N/64 tiles are dealt to the C ranks as evenly as possible (at most NGB each)
     const int base_t = NW / C, rem_t = NW % C;
@@ -335,7 +335,8 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                                   (long long)it.rb * p.lR;
                 const float* dp_ = Dws + (lp - LSE);
                 const unsigned long long* mp = maskbits ? maskbits + ((long long)it.b * p.R + it.rb) * NW + tile : nullptr;
-                float lse_n = __ldg(lp), dd_n = __ldg(dp_);
+                const bool inq = it.q0 + row < N;  // queries beyond N (last, partial block): LSE = -inf makes p = dS = 0
+                float lse_n = inq ? __ldg(lp) : -INFINITY, dd_n = inq ? __ldg(dp_) : 0.0f;
                 uint64_t mb_n = mp ? ldg_u64(mp) : ~0ull;
                 // my row of the bias tile -> registers for the whole item; the shared buffer goes back to the producer
                 mbar_wait(bias_full, il & 1);
@@ -353,8 +354,10 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     const uint64_t mb = mb_n;
                     if (r + 1 < NR) {
                         lp += p.lR; dp_ += p.lR;
-                        lse_n = __ldg(lp);
-                        dd_n = __ldg(dp_);
+                        if (inq) {
+                            lse_n = __ldg(lp);
+                            dd_n = __ldg(dp_);
+                        }
                         if (mp) { mp += NW; mb_n = ldg_u64(mp); }
                     }
 #pragma unroll
@@ -399,18 +402,24 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     acc2[i] = pack2(0.0f, 0.0f);
                 }
                 const int bh = it.b * p.H + it.h;
-                if (G > 1) {
+                const int nk = N - tile * BK;  // keys of my tile that exist (>= BK except in the last tile; N % 8 == 0)
+                if (!inq) {
+                    // query row beyond N: nothing to store
+                } else if (G > 1) {
                     float* out = planes + ((long long)(it.rb / NR) * p.B * p.H + bh) * N * N + (long long)(it.q0 + row) * N + tile * BK;
 #pragma unroll
-                    for (int i = 0; i < BK; i += 4) *(float4*)(out + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
+                    for (int i = 0; i < BK; i += 4)
+                        if (i < nk) *(float4*)(out + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
                 } else {
                     float* out = dBias + (long long)bh * N * N + (long long)(it.q0 + row) * p.bQ + (long long)(tile * BK) * p.bK;
                     if (p.bK == 1) {
 #pragma unroll
-                        for (int i = 0; i < BK; i += 4) *(float4*)(out + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
+                        for (int i = 0; i < BK; i += 4)
+                            if (i < nk) *(float4*)(out + i) = make_float4(acc[i], acc[i + 1], acc[i + 2], acc[i + 3]);
                     } else {
 #pragma unroll
-                        for (int i = 0; i < BK; ++i) out[(long long)i * p.bK] = acc[i];
+                        for (int i = 0; i < BK; ++i)
+                            if (i < nk) out[(long long)i * p.bK] = acc[i];
                     }
                 }
             }
@@ -464,7 +473,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
                         st_async_v4(dst + ((i ^ sw) << 4), f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3], infull_next + j * 8);
-                } else {  // last rank: dQ = scale * sum
+                } else if (it.q0 + row < N) {  // last rank: dQ = scale * sum (queries beyond N: nothing to store)
                     uint4* pq = (uint4*)qp;
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
@@ -487,7 +496,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 
 // cluster size for N/64 key tiles at <= NGB tiles per rank, from the sizes the launch code accepts
 int sm100_dqdb_cluster(int N) {
-    const int T = N / BK, need = (T + NGB - 1) / NGB;
+    const int T = (N + BK - 1) / BK, need = (T + NGB - 1) / NGB;
     const int sizes[] = {1, 2, 3, 4, 6, 8, 12, 16};
     for (int s : sizes)
         if (s >= need) return s;
@@ -515,7 +524,7 @@ bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
         cudaGetLastError();
         return false;
     }
-    const long long base = (long long)p.B * p.H * (p.N / BQ);
+    const long long base = (long long)p.B * p.H * ((p.N + BQ - 1) / BQ);
     int bestG = 1;
     double best = 1e30;
     for (int G = 1; G <= kDqdbMaxSplit; ++G) {
@@ -548,7 +557,7 @@ tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const voi
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = (unsigned)C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    const int n_items = p.B * p.H * (p.N / BQ) * G;
+    const int n_items = p.B * p.H * ((p.N + BQ - 1) / BQ) * G;
     {
         ProfScope ps("sm100_dqdb_kernel", st);
         TRI_CUDA_CHECK(cudaLaunchKernelEx(&cfg, sm100_dqdb_kernel, tQ, tA, tK, tV, tB, p, maskbits, LSE, Dws, (__nv_bfloat16*)dQ,

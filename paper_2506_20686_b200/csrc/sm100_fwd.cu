@@ -57,7 +57,7 @@ struct Item { int b, h, q0, r4; };
 // row quad fastest (measured: query block fastest halves the K / V re-reads from HBM but is 4 % slower at cfg5, where
 // the ending-node rows are 64-byte neighbours in memory and concurrent quads share DRAM pages)
 __device__ __forceinline__ Item decode_item(int item, int N, int H, int R) {
-    const int NRQ = R / NG, NQB = N / BQ;
+    const int NRQ = R / NG, NQB = (N + BQ - 1) / BQ;
     Item it;
     it.r4 = (item % NRQ) * NG;
     int t = item / NRQ;
@@ -93,7 +93,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
 
     const int tid = threadIdx.x, warp = tid >> 5;
     const int N = p.N;
-    const int TPR = N / BK;  // key tiles per row
+    const int TPR = (N + BK - 1) / BK;  // key tiles per row (the last one may be partial: TMA zero-fills, the mask bits hide it)
     const int n_items = (total_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     const int NT_all = n_items * TPR;  // tiles per group over the CTA's life
 
@@ -200,7 +200,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         const uint32_t tS = tmem + g * 128 + lane_off, tP = tS + 64, tO = tS + 96;
         const float sl = rsqrtf((float)DH) * kLog2e;  // scores are kept in log2 units: x = S * scale * log2e + log2e * bias
         const uint64_t sl2 = pack2(sl, sl);
-        const int NW = N / 64;  // mask words per row
+        const int NW = (N + 63) / 64;  // mask words per row
         int bst = 0, bph = 0;
         int n = 0;
         uint64_t* my_tok = tok + g * 4 + (warp & 3);
@@ -305,10 +305,11 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 warp_arrive(p_ready + g);
             }
             // ---- row epilogue: O = sigmoid(G) * O_r / l ; LSE = m + ln l -------------------------------
+            const bool inq = it.q0 + row < N;  // the last query block may be partial
             uint4 gv[4];
             const uint4* gp = (const uint4*)(G + off);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) gv[j] = __ldg(gp + j);
+            for (int j = 0; j < 4; ++j) gv[j] = inq ? __ldg(gp + j) : make_uint4(0u, 0u, 0u, 0u);
             mbar_wait(pv_done + g, (n - 1) & 1);
             tc_fence_after();
             uint32_t o[32];
@@ -326,10 +327,10 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                     const float s0 = __fdividef(1.0f, 1.0f + ex2(-g0 * kLog2e)), s1 = __fdividef(1.0f, 1.0f + ex2(-g1 * kLog2e));
                     ow[e] = pack_bf16(__uint_as_float(o[j * 8 + 2 * e]) * inv * s0, __uint_as_float(o[j * 8 + 2 * e + 1]) * inv * s1);
                 }
-                op[j] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+                if (inq) op[j] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
             const long long loff = (long long)it.b * p.lB + (long long)it.h * N + (long long)r * p.lR + (long long)(it.q0 + row) * p.lQ;
-            LSE[loff] = l_run > 0.0f ? m_run * kLn2 + __logf(l_run) : -INFINITY;
+            if (inq) LSE[loff] = l_run > 0.0f ? m_run * kLn2 + __logf(l_run) : -INFINITY;
         }
     }
     tc_fence_before();
@@ -342,10 +343,12 @@ __global__ void transpose_bf16_kernel(const __nv_bfloat16* __restrict__ in, __nv
     __shared__ __nv_bfloat16 tile[32][33];
     const long long plane = (long long)blockIdx.z * N * N;
     const int x = blockIdx.x * 32 + threadIdx.x, y0 = blockIdx.y * 32;
-    for (int j = threadIdx.y; j < 32; j += 8) tile[j][threadIdx.x] = in[plane + (long long)(y0 + j) * N + x];
+    for (int j = threadIdx.y; j < 32; j += 8)
+        if (x < N && y0 + j < N) tile[j][threadIdx.x] = in[plane + (long long)(y0 + j) * N + x];
     __syncthreads();
     const int xo = blockIdx.y * 32 + threadIdx.x, yo0 = blockIdx.x * 32;
-    for (int j = threadIdx.y; j < 32; j += 8) out[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
+    for (int j = threadIdx.y; j < 32; j += 8)
+        if (xo < N && yo0 + j < N) out[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
 }
 
 // fp32 planes of f * bias for the softmax warps (no bf16 unpacking in the inner loops): nat[bh][y][x] = f*in[bh][y][x],
@@ -356,6 +359,7 @@ __global__ void bias_planes_kernel(const __nv_bfloat16* __restrict__ in, float* 
     const long long plane = (long long)blockIdx.z * N * N;
     const int x = blockIdx.x * 32 + threadIdx.x, y0 = blockIdx.y * 32;
     for (int j = threadIdx.y; j < 32; j += 8) {
+        if (x >= N || y0 + j >= N) continue;
         const float v = f * __bfloat162float(in[plane + (long long)(y0 + j) * N + x]);
         if (nat) nat[plane + (long long)(y0 + j) * N + x] = v;
         tile[j][threadIdx.x] = v;
@@ -363,19 +367,22 @@ __global__ void bias_planes_kernel(const __nv_bfloat16* __restrict__ in, float* 
     if (!tr) return;
     __syncthreads();
     const int xo = blockIdx.y * 32 + threadIdx.x, yo0 = blockIdx.x * 32;
-    for (int j = threadIdx.y; j < 32; j += 8) tr[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
+    for (int j = threadIdx.y; j < 32; j += 8)
+        if (xo < N && yo0 + j < N) tr[plane + (long long)(yo0 + j) * N + xo] = tile[threadIdx.x][j];
 }
 
 // keep flags [B,N,N] (u8) -> one 64-bit word per (b, row r, 64-key tile): bit k = key 64*w + k of row r is visible.
 // Rows / keys follow the variant (mask element (r,k) at r*mR + k*mK), so the kernels read one word per tile.
+// Keys >= N of the last (partial) tile get a zero bit; mask == nullptr packs "every key < N visible" (ragged N only).
 __global__ void __launch_bounds__(128) pack_mask_kernel(const unsigned char* __restrict__ mask,
                                                         unsigned long long* __restrict__ bits, Problem p) {
     const int lane = threadIdx.x & 31, w = blockIdx.x * 4 + (threadIdx.x >> 5);
-    const int r = blockIdx.y, b = blockIdx.z, NW = p.N / 64;
+    const int r = blockIdx.y, b = blockIdx.z, NW = (p.N + 63) / 64;
     if (w >= NW) return;
-    const unsigned char* base = mask + (long long)b * p.mB + (long long)r * p.mR;
-    const unsigned lo = __ballot_sync(0xffffffffu, base[(long long)(w * 64 + lane) * p.mK] != 0);
-    const unsigned hi = __ballot_sync(0xffffffffu, base[(long long)(w * 64 + 32 + lane) * p.mK] != 0);
+    const unsigned char* base = mask ? mask + (long long)b * p.mB + (long long)r * p.mR : nullptr;
+    const int k_lo = w * 64 + lane, k_hi = k_lo + 32;
+    const unsigned lo = __ballot_sync(0xffffffffu, k_lo < p.N && (!base || base[(long long)k_lo * p.mK] != 0));
+    const unsigned hi = __ballot_sync(0xffffffffu, k_hi < p.N && (!base || base[(long long)k_hi * p.mK] != 0));
     if (lane == 0) bits[((long long)b * p.R + r) * NW + w] = (unsigned long long)lo | ((unsigned long long)hi << 32);
 }
 
@@ -393,30 +400,36 @@ int sm_count() {
 
 tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cudaStream_t st) {
     ProfScope ps("transpose_bf16_kernel", st);
-    transpose_bf16_kernel<<<dim3(N / 32, N / 32, BH), dim3(32, 8), 0, st>>>((const __nv_bfloat16*)in, (__nv_bfloat16*)out, N);
+    transpose_bf16_kernel<<<dim3((N + 31) / 32, (N + 31) / 32, BH), dim3(32, 8), 0, st>>>((const __nv_bfloat16*)in, (__nv_bfloat16*)out, N);
     return TRI_OK;
 }
 
 tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int N, float f, cudaStream_t st) {
     ProfScope ps("bias_planes_kernel", st);
-    bias_planes_kernel<<<dim3(N / 32, N / 32, BH), dim3(32, 8), 0, st>>>((const __nv_bfloat16*)in, nat, tr, N, f);
+    bias_planes_kernel<<<dim3((N + 31) / 32, (N + 31) / 32, BH), dim3(32, 8), 0, st>>>((const __nv_bfloat16*)in, nat, tr, N, f);
     return TRI_OK;
 }
 
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st) {
     ProfScope ps("pack_mask_kernel", st);
-    pack_mask_kernel<<<dim3((p.N / 64 + 3) / 4, p.R, p.B), 128, 0, st>>>(mask, (unsigned long long*)bits, p);
+    pack_mask_kernel<<<dim3(((p.N + 63) / 64 + 3) / 4, p.R, p.B), 128, 0, st>>>(mask, (unsigned long long*)bits, p);
     return TRI_OK;
 }
 
 int sm100_sm_count() { return sm_count(); }
 
-// N <= 2048: the fused dQ + dBias stage needs one cluster rank per two 64-key tiles (<= 16 ranks)
+// N <= 2048: the fused dQ + dBias stage needs one cluster rank per two 64-key tiles (<= 16 ranks).  N % 8 == 0: the
+// bias planes are read by TMA (16-byte row pitch in bf16).  N need not be a multiple of the 64 / 128-position tiles: TMA
+// zero-fills what lies beyond N, the packed mask hides keys >= N, stores of queries / keys >= N are predicated off.
 bool sm100_supported(const Problem& p, tri_dtype dt) {
-    return dt == TRI_BF16 && p.d == 32 && p.N % 128 == 0 && p.N <= 2048 && p.R % 4 == 0 && (p.R == p.N || p.variant == TRI_STARTING);
+    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 2048 && p.R % 4 == 0 &&
+           (p.R == p.N || p.variant == TRI_STARTING);
 }
 
-size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.R * (p.N / 64) * 8, 256); }
+// the kernels need the packed mask words when the caller passed a mask or when the last 64-key tile is partial
+bool sm100_needs_maskbits(const Problem& p, const unsigned char* mask) { return mask != nullptr || p.N % 64 != 0; }
+
+size_t sm100_maskbits_bytes(const Problem& p) { return align_up((size_t)p.B * p.R * ((p.N + 63) / 64) * 8, 256); }
 
 size_t sm100_fwd_workspace(const Problem& p) {
     return sm100_maskbits_bytes(p) + align_up((size_t)p.B * p.H * p.N * p.N * 4, 256);  // + log2e * bias[q][k], fp32
@@ -425,7 +438,7 @@ size_t sm100_fwd_workspace(const Problem& p) {
 tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void* V, const void* G, const void* bias,
                      const unsigned char* mask, void* O, float* LSE, void* ws, cudaStream_t st) {
     void* maskbits = nullptr;
-    if (mask) {
+    if (sm100_needs_maskbits(p, mask)) {
         maskbits = ws;
         tri_status s = sm100_pack_mask(p, mask, maskbits, st);
         if (s != TRI_OK) return s;
@@ -445,7 +458,7 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
     TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));
-    const long long items = (long long)p.B * p.H * (p.N / BQ) * (p.R / NG);
+    const long long items = (long long)p.B * p.H * ((p.N + BQ - 1) / BQ) * (p.R / NG);
     const int grid = (int)(items < sm_count() ? items : sm_count());
     {
         ProfScope ps("sm100_fwd_kernel", st);

@@ -97,6 +97,7 @@ tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int 
 // keep flags -> one 64-bit word per (b, row, 64-key tile), rows / keys in the variant's sense
 tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bits, cudaStream_t st);
 size_t sm100_maskbits_bytes(const Problem& p);
+bool sm100_needs_maskbits(const Problem& p, const unsigned char* mask);
 // dK / dV stage (sm100_dkdv.cu): NL / ND are fp32 [B,N,H,N] scratch arrays of sm100_dkdv2_aux_bytes() each, filled by
 // sm100_lse_prep; a launch covers work items [item_begin, item_begin + item_count) of sm100_dkdv2_items() on <= max_ctas CTAs
 size_t sm100_dkdv2_aux_bytes(const Problem& p);

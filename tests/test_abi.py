@@ -84,7 +84,9 @@ def test_overlapping_outputs_are_rejected_before_any_launch(lib):
 
 def test_tensor_core_path_query(lib):
     assert lib.tri_attn_uses_tensor_cores(2, 768, 4, 32, 0, 1) == 1
-    assert lib.tri_attn_uses_tensor_cores(1, 200, 4, 32, 0, 1) == 0   # N not a multiple of 128: CUDA-core kernels
+    assert lib.tri_attn_uses_tensor_cores(1, 200, 4, 32, 0, 1) == 1   # N % 8 == 0 is enough (partial tiles are masked)
+    assert lib.tri_attn_uses_tensor_cores(1, 204, 4, 32, 0, 1) == 0   # N % 8 != 0: CUDA-core kernels
+    assert lib.tri_attn_uses_tensor_cores(1, 120, 4, 32, 0, 1) == 0   # N < 128: CUDA-core kernels
     assert lib.tri_attn_uses_tensor_cores(1, 128, 4, 64, 0, 1) == 0   # d != 32
     assert lib.tri_attn_uses_tensor_cores(1, 128, 4, 32, 0, 0) == 0   # fp32 (reading A14)
 
