@@ -100,7 +100,10 @@ BwdWs bwd_ws_layout(const Problem& p) {
 // one side stream + fork / join events per device (created on first use, never destroyed)
 struct SideStream {
     cudaStream_t stream = nullptr;
-    cudaEvent_t fork = nullptr, join = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;    // stage-1 slice beside stage 2
+    cudaEvent_t fork0 = nullptr, join0 = nullptr;  // bias / mask preparation beside the pre-process kernel
+    cudaStream_t hi = nullptr;                     // high-priority stream of the dBias plane reduction
+    cudaEvent_t stage2 = nullptr, join2 = nullptr; // stage 2 done -> reduction (beside the rest of stage 1) -> joined
     bool ready = false;
 };
 std::mutex g_side_mu;
@@ -114,6 +117,13 @@ SideStream* side_stream() {
         if (cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) != cudaSuccess) return nullptr;
         if (cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming) != cudaSuccess) return nullptr;
         if (cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.fork0, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.join0, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.stage2, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        if (cudaEventCreateWithFlags(&s.join2, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        int lo = 0, hi = 0;  // numerically lower = higher priority
+        if (cudaDeviceGetStreamPriorityRange(&lo, &hi) != cudaSuccess) return nullptr;
+        if (cudaStreamCreateWithPriority(&s.hi, cudaStreamNonBlocking, hi) != cudaSuccess) return nullptr;
         s.ready = true;
     }
     return &s;
@@ -136,13 +146,22 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     void* dA = (char*)ws + w.da_off;
     void* biasT = (char*)ws + w.biast_off;
     const long long rows = (long long)p.B * p.R * p.H * p.N;
+    // Library-owned side stream, forked from and joined back into `st` with events (to the caller the call is one unit of
+    // work on `st`).  It carries (1) the bias / mask preparation, which is independent of the HBM-bound pre-process kernel,
+    // (2) a slice of stage 1 beside stage 2, (3) the dBias plane reduction beside the rest of stage 1.
+    SideStream* side = side_stream();
+    cudaStream_t sp = side ? side->stream : st;  // where the preparation kernels go
+    if (side) {
+        TRI_CUDA_CHECK(cudaEventRecord(side->fork0, st));
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(side->stream, side->fork0, 0));
+    }
     {
         ProfScope ps("sm100_bwd_pre_kernel", st);
         sm100_bwd_pre_kernel<<<(unsigned)((rows * 4 + 255) / 256), 256, 0, st>>>(rows, (const uint4*)dO, (const uint4*)O,
                                                                                (const uint4*)G, (uint4*)dG, (uint4*)dA, Dws);
     }
     TRI_LAUNCH_CHECK("sm100_bwd_pre_kernel");
-    tri_status s = sm100_transpose_planes(bias, biasT, p.B * p.H, p.N, st);
+    tri_status s = sm100_transpose_planes(bias, biasT, p.B * p.H, p.N, sp);
     if (s != TRI_OK) return s;
     TRI_LAUNCH_CHECK("sm100_transpose_bf16");
     const void* bias_kq = p.variant == TRI_STARTING ? biasT : bias;  // [k][q]
@@ -150,22 +169,25 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     unsigned long long* maskbits = nullptr;
     if (sm100_needs_maskbits(p, mask)) {
         maskbits = (unsigned long long*)((char*)ws + w.mask_off);
-        if ((s = sm100_pack_mask(p, mask, maskbits, st)) != TRI_OK) return s;
+        if ((s = sm100_pack_mask(p, mask, maskbits, sp)) != TRI_OK) return s;
         TRI_LAUNCH_CHECK("pack_mask_kernel");
+    }
+    float* biasL = (float*)((char*)ws + w.biasl_off);
+    {
+        const bool tr = p.variant == TRI_ENDING;
+        if ((s = sm100_bias_planes(bias, tr ? nullptr : biasL, tr ? biasL : nullptr, p.B * p.H, p.N, kLog2e, sp)) != TRI_OK) return s;
+        TRI_LAUNCH_CHECK("bias_planes_kernel");
+    }
+    if (side) {
+        TRI_CUDA_CHECK(cudaEventRecord(side->join0, side->stream));
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(st, side->join0, 0));
     }
     float* NL = (float*)((char*)ws + w.nl_off);
     float* ND = (float*)((char*)ws + w.nd_off);
     if ((s = sm100_lse_prep(p, LSE, Dws, NL, ND, st)) != TRI_OK) return s;
-    float* biasL = (float*)((char*)ws + w.biasl_off);
-    {
-        const bool tr = p.variant == TRI_ENDING;
-        if ((s = sm100_bias_planes(bias, tr ? nullptr : biasL, tr ? biasL : nullptr, p.B * p.H, p.N, kLog2e, st)) != TRI_OK) return s;
-        TRI_LAUNCH_CHECK("bias_planes_kernel");
-    }
     // Stage 2 (dQ + dBias, one recomputation of P / dS) runs as clusters and leaves some SMs empty (132 of 148 at N = 768:
     // cudaOccupancyMaxActiveClusters).  Stage 1 (dK, dV) is independent of it, so a first slice of stage 1's work items runs
-    // on those SMs at the same time, on a library-owned side stream forked from and joined back into `st` with events;
-    // the rest of stage 1 follows on all SMs.
+    // on those SMs at the same time on the side stream; the rest of stage 1 follows on all SMs.
     float* planes = (float*)((char*)ws + w.planes_off);
     int Gs = 1, C2 = 0, grid2 = 0;
     if (!sm100_dqdb_plan(p, &C2, &Gs, &grid2)) return cuda_fail(cudaErrorLaunchFailure, "sm100_dqdb_plan: no resident cluster of the needed size");
@@ -173,13 +195,11 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     const int sms = sm100_sm_count();
     const int spare = sms - grid2;
     long long itemsA = 0;
-    SideStream* side = nullptr;
-    if (spare >= 4 && items1 > 4 * sms) {
+    if (side && spare >= 4 && items1 > 4 * sms) {
         // the spare SMs work for about the duration of stage 2, which is ~1.4x stage 1's on the whole chip
         itemsA = (long long)((double)items1 * spare / sms * 1.4);
-        side = side_stream();
-        if (!side) itemsA = 0;
     }
+    const bool reduce = Gs > 1 || accumulate_dbias;
     if (itemsA > 0) {
         TRI_CUDA_CHECK(cudaEventRecord(side->fork, st));
         TRI_CUDA_CHECK(cudaStreamWaitEvent(side->stream, side->fork, 0));
@@ -190,20 +210,32 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
         if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, NL, ND, dK, dV, 0, itemsA, spare, "sm100_dkdv_kernel(side)",
                                     side->stream)) != TRI_OK)
             return s;
-        TRI_CUDA_CHECK(cudaEventRecord(side->join, side->stream));
+    }
+    if (reduce) {
+        // level 2 of the dBias reduction needs stage 2 only.  On a high-priority stream its (small, memory-bound) blocks
+        // take the SMs that stage 2 frees ahead of the persistent CTAs of the rest of stage 1, and finish beside them;
+        // enqueued behind stage 1 they would wait for its last CTA.
+        cudaStream_t sr = side ? side->hi : st;
+        if (side) {
+            TRI_CUDA_CHECK(cudaEventRecord(side->stage2, st));
+            TRI_CUDA_CHECK(cudaStreamWaitEvent(side->hi, side->stage2, 0));
+        }
+        {
+            ProfScope ps("sm100_dbias_reduce_kernel", sr);
+            sm100_dbias_reduce_kernel<<<dim3((p.N + 31) / 32, (p.N + 31) / 32, p.B * p.H), 256, 0, sr>>>(
+                planes, dBias, p.B * p.H, p.N, Gs, p.variant == TRI_ENDING ? 1 : 0, accumulate_dbias ? 1 : 0);
+        }
+        TRI_LAUNCH_CHECK("sm100_dbias_reduce_kernel");
+        if (side) TRI_CUDA_CHECK(cudaEventRecord(side->join2, side->hi));
     }
     if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, NL, ND, dK, dV, itemsA, items1 - itemsA, sms, "sm100_dkdv_kernel", st)) !=
         TRI_OK)
         return s;
-    if (itemsA > 0) TRI_CUDA_CHECK(cudaStreamWaitEvent(st, side->join, 0));
-    if (Gs > 1 || accumulate_dbias) {
-        {
-            ProfScope ps("sm100_dbias_reduce_kernel", st);
-            sm100_dbias_reduce_kernel<<<dim3((p.N + 31) / 32, (p.N + 31) / 32, p.B * p.H), 256, 0, st>>>(
-                planes, dBias, p.B * p.H, p.N, Gs, p.variant == TRI_ENDING ? 1 : 0, accumulate_dbias ? 1 : 0);
-        }
-        TRI_LAUNCH_CHECK("sm100_dbias_reduce_kernel");
+    if (itemsA > 0) {
+        TRI_CUDA_CHECK(cudaEventRecord(side->join, side->stream));
+        TRI_CUDA_CHECK(cudaStreamWaitEvent(st, side->join, 0));
     }
+    if (side && reduce) TRI_CUDA_CHECK(cudaStreamWaitEvent(st, side->join2, 0));
     return TRI_OK;
 }
 

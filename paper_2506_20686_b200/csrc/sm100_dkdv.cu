@@ -56,9 +56,10 @@ struct DkdvSmem {
 struct ItemK { int b, h, k0, r0; };
 // key block fastest: the CTAs that run concurrently share the Q / dA rows of a few row triples (read once from HBM,
 // then from L2) instead of streaming the whole pair tensor once per key block
+template <bool kAligned>
 __device__ __forceinline__ ItemK decode_itemk(int item, int N, int H, int NT3) {
     ItemK it;
-    const int NKB = (N + BKEY - 1) / BKEY;
+    const int NKB = kAligned ? N / BKEY : (N + BKEY - 1) / BKEY;
     it.k0 = (item % NKB) * BKEY;
     int t = item / NKB;
     it.r0 = (t % NT3) * NGK;
@@ -97,6 +98,8 @@ __device__ __forceinline__ void dkdv_chunk(const uint32_t (&sr)[16], const uint3
     }
 }
 
+// kAligned: N % 128 == 0 (no partial tile anywhere: the bounds checks fold away)
+template <bool kAligned>
 __global__ void __launch_bounds__(DKDV_THREADS, 1)
 sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmA,
                    const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
@@ -121,9 +124,9 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
     uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int N = p.N, NW = (N + 63) / 64;
+    const int N = p.N, NW = kAligned ? N / 64 : (N + 63) / 64;
     const int NT3 = (p.R + NGK - 1) / NGK;  // row triples (the last one may be partial)
-    const int NS = (N + BQS - 1) / BQS;   // ring stages per row (the last one may be partial: TMA zero-fills Q / dA / bias^T,
+    const int NS = kAligned ? N / BQS : (N + BQS - 1) / BQS;   // ring stages per row (the last one may be partial: TMA zero-fills Q / dA / bias^T,
                                           // NL is -inf there, so P^T = dS^T = 0 for queries >= N;
                                           // NL / ND rows are padded to NS * BQS by lse_prep_kernel)
     const int n_items = (total_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
@@ -152,7 +155,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             // ---- TMA producer ----
             int n = 0;  // stage counter over the CTA's life
             for (int il = 0; il < n_items; ++il) {
-                const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
+                const ItemK it = decode_itemk<kAligned>(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
                 const int bh = it.b * p.H + it.h;
                 const int nr = min(NGK, p.R - it.r0);  // active rows of the item
                 if (il > 0) mbar_wait(kv_free, (il - 1) & 1);
@@ -194,7 +197,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
             int un = 0;  // unit counter (barrier phases of s_full / p_ready)
             int ia = 0;  // rows this group has processed (barrier phases of acc_full / acc_free)
             for (int il = 0; il < n_items; ++il) {
-                const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
+                const ItemK it = decode_itemk<kAligned>(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
                 const bool active = it.r0 + g < p.R;
                 mbar_wait(kv_full, il & 1);
                 tc_fence_after();
@@ -290,10 +293,10 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
         uint64_t* my_tok = tok + g * 4 + (warp & 3);
         uint64_t* next_tok = tok + ((g + 1) % NGK) * 4 + (warp & 3);
         for (int il = 0; il < n_items; ++il) {
-            const ItemK it = decode_itemk(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
+            const ItemK it = decode_itemk<kAligned>(item_begin + (int)blockIdx.x + il * (int)gridDim.x, N, p.H, NT3);
             const int r = it.r0 + g;
             const bool active = r < p.R;
-            bool keep = it.k0 + row < N;  // keys beyond N of the last (partial) key block are TMA zero-fill
+            bool keep = kAligned || it.k0 + row < N;  // keys beyond N of the last (partial) key block are TMA zero-fill
             if (active && keep && maskbits)
                 keep = (ldg_u64(maskbits + ((long long)it.b * p.R + r) * NW + (it.k0 + row) / 64) >> ((it.k0 + row) & 63)) & 1ull;
             const bool allkeep = __all_sync(0xffffffffu, keep);
@@ -362,7 +365,7 @@ sm100_dkdv2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constan
                 const long long off = (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)r * p.sSlice + (long long)(it.k0 + row) * p.sPos;
                 uint4* pv = (uint4*)(dV + off);
                 uint4* pk = (uint4*)(dK + off);
-                if (it.k0 + row >= N) continue;  // keys beyond N of the last (partial) key block: nothing to store
+                if (!kAligned && it.k0 + row >= N) continue;  // keys beyond N of the last (partial) key block: nothing to store
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     uint32_t a[4], c[4];
@@ -433,12 +436,13 @@ tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, c
         !make_tmap_u(&tK, K, p.B, p.N, p.H, p.d, p.variant, BKEY, p.R) || !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BKEY, p.R) ||
         !make_tmap_plane(&tB, bias_kq, p.B * p.H, p.N, BKEY))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
-    TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_dkdv2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DkdvSmem::total));
+    auto kern = p.N % 128 == 0 ? sm100_dkdv2_kernel<true> : sm100_dkdv2_kernel<false>;
+    TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, DkdvSmem::total));
     const int grid = (int)(item_count < max_ctas ? item_count : max_ctas);
     {
         ProfScope ps(prof_name, st);
-        sm100_dkdv2_kernel<<<grid, DKDV_THREADS, DkdvSmem::total, st>>>(tQ, tA, tK, tV, tB, p, maskbits, NL, ND, (__nv_bfloat16*)dK,
-                                                                       (__nv_bfloat16*)dV, (int)item_begin, (int)item_count);
+        kern<<<grid, DKDV_THREADS, DkdvSmem::total, st>>>(tQ, tA, tK, tV, tB, p, maskbits, NL, ND, (__nv_bfloat16*)dK, (__nv_bfloat16*)dV,
+                                                          (int)item_begin, (int)item_count);
     }
     TRI_LAUNCH_CHECK("sm100_dkdv_kernel");
     return TRI_OK;

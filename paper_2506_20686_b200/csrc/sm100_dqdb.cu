@@ -126,9 +126,10 @@ __device__ __forceinline__ void dqdb_chunk(const uint32_t (&sr)[16], const uint3
 
 struct Item2 { int b, h, q0, rb; };
 // query block fastest: clusters that run concurrently work on the same rows (K_r, V_r shared through L2)
+template <bool kAligned>
 __device__ __forceinline__ Item2 decode_item2(int item, int N, int H, int G, int NR) {
     Item2 it;
-    const int NQB = (N + BQ - 1) / BQ;
+    const int NQB = kAligned ? N / BQ : (N + BQ - 1) / BQ;
     it.q0 = (item % NQB) * BQ;
     int t = item / NQB;
     it.rb = (t % G) * NR;
@@ -138,6 +139,8 @@ __device__ __forceinline__ Item2 decode_item2(int item, int N, int H, int G, int
     return it;
 }
 
+// kAligned: N % 128 == 0 (no partial tile anywhere: the bounds checks fold away)
+template <bool kAligned>
 __global__ void __launch_bounds__(DQDB_THREADS, 1)
 sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmA,
                   const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
@@ -169,7 +172,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     uint32_t* tmem_slot = (uint32_t*)(bars + L::n_bars);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int N = p.N, NW = (N + BK - 1) / BK;  // the last tile / query block may be partial (TMA zero-fill + mask bits)
+    const int N = p.N, NW = kAligned ? N / BK : (N + BK - 1) / BK;  // the last tile / query block may be partial (TMA zero-fill + mask bits)
     const int C = (int)cluster_nctarank(), c = (int)cluster_ctarank();
     // key tiles of this rank: the N/64 tiles are dealt to the C ranks as evenly as possible (at most NGB each)
     const int base_t = NW / C, rem_t = NW % C;
@@ -226,7 +229,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             };
             int n = 0;
             for (int il = 0; il < n_my; ++il) {
-                const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
+                const Item2 it = decode_item2<kAligned>(cid + il * ncl, N, p.H, G, NR);
                 const int bh = it.b * p.H + it.h;
                 if (il > 0) mbar_wait(bias_free, (il - 1) & 1);
                 if (elect_one()) {
@@ -330,12 +333,12 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             for (int i = 0; i < BK / 2; ++i) acc2[i] = pack2(0.0f, 0.0f);
             int n = 0;
             for (int il = 0; il < n_my; ++il) {
-                const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
+                const Item2 it = decode_item2<kAligned>(cid + il * ncl, N, p.H, G, NR);
                 const float* lp = LSE + (long long)it.b * p.lB + (long long)it.h * N + (long long)(it.q0 + row) * p.lQ +
                                   (long long)it.rb * p.lR;
                 const float* dp_ = Dws + (lp - LSE);
                 const unsigned long long* mp = maskbits ? maskbits + ((long long)it.b * p.R + it.rb) * NW + tile : nullptr;
-                const bool inq = it.q0 + row < N;  // queries beyond N (last, partial block): LSE = -inf makes p = dS = 0
+                const bool inq = kAligned || it.q0 + row < N;  // queries beyond N (last, partial block): LSE = -inf makes p = dS = 0
                 float lse_n = inq ? __ldg(lp) : -INFINITY, dd_n = inq ? __ldg(dp_) : 0.0f;
                 uint64_t mb_n = mp ? ldg_u64(mp) : ~0ull;
                 // my row of the bias tile -> registers for the whole item; the shared buffer goes back to the producer
@@ -402,7 +405,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     acc2[i] = pack2(0.0f, 0.0f);
                 }
                 const int bh = it.b * p.H + it.h;
-                const int nk = N - tile * BK;  // keys of my tile that exist (>= BK except in the last tile; N % 8 == 0)
+                const int nk = kAligned ? BK : N - tile * BK;  // keys of my tile that exist (>= BK except in the last tile; N % 8 == 0)
                 if (!inq) {
                     // query row beyond N: nothing to store
                 } else if (G > 1) {
@@ -438,7 +441,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
             for (int i = 0; i < NIN && i < NRtot; ++i) mbar_expect_tx(in_full + i, INBOX_BYTES);
         int n = 0;
         for (int il = 0; il < n_my; ++il) {
-            const Item2 it = decode_item2(cid + il * ncl, N, p.H, G, NR);
+            const Item2 it = decode_item2<kAligned>(cid + il * ncl, N, p.H, G, NR);
             __nv_bfloat16* qp = dQ + (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)it.rb * p.sSlice + (long long)(it.q0 + row) * p.sPos;
             for (int r = 0; r < NR; ++r, ++n, qp += p.sSlice) {
                 const int j = n & 1, ph = (n >> 1) & 1;  // inbox slot and its phase
@@ -473,7 +476,7 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
                         st_async_v4(dst + ((i ^ sw) << 4), f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3], infull_next + j * 8);
-                } else if (it.q0 + row < N) {  // last rank: dQ = scale * sum (queries beyond N: nothing to store)
+                } else if (kAligned || it.q0 + row < N) {  // last rank: dQ = scale * sum (queries beyond N: nothing to store)
                     uint4* pq = (uint4*)qp;
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
@@ -509,8 +512,9 @@ int sm100_dqdb_cluster(int N) {
 bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
     const int C = sm100_dqdb_cluster(p.N);
     if (C == 0) return false;
-    if (cudaFuncSetAttribute(sm100_dqdb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DqdbSmem::total) != cudaSuccess) return false;
-    if (C > 8 && cudaFuncSetAttribute(sm100_dqdb_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return false;
+    auto kern = p.N % 128 == 0 ? sm100_dqdb_kernel<true> : sm100_dqdb_kernel<false>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, DqdbSmem::total) != cudaSuccess) return false;
+    if (C > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return false;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(C * 64));
     cfg.blockDim = dim3(DQDB_THREADS);
@@ -520,7 +524,7 @@ bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
     at[0].val.clusterDim.x = (unsigned)C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
     int ncl = 0;
-    if (cudaOccupancyMaxActiveClusters(&ncl, sm100_dqdb_kernel, &cfg) != cudaSuccess || ncl <= 0) {
+    if (cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg) != cudaSuccess || ncl <= 0) {
         cudaGetLastError();
         return false;
     }
@@ -560,7 +564,7 @@ tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const voi
     const int n_items = p.B * p.H * ((p.N + BQ - 1) / BQ) * G;
     {
         ProfScope ps("sm100_dqdb_kernel", st);
-        TRI_CUDA_CHECK(cudaLaunchKernelEx(&cfg, sm100_dqdb_kernel, tQ, tA, tK, tV, tB, p, maskbits, LSE, Dws, (__nv_bfloat16*)dQ,
+        TRI_CUDA_CHECK(cudaLaunchKernelEx(&cfg, p.N % 128 == 0 ? sm100_dqdb_kernel<true> : sm100_dqdb_kernel<false>, tQ, tA, tK, tV, tB, p, maskbits, LSE, Dws, (__nv_bfloat16*)dQ,
                                           dBias, planes, G, n_items, kbox));
     }
     TRI_LAUNCH_CHECK("sm100_dqdb_kernel");

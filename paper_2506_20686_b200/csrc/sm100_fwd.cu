@@ -56,8 +56,9 @@ struct FwdSmem {
 struct Item { int b, h, q0, r4; };
 // row quad fastest (measured: query block fastest halves the K / V re-reads from HBM but is 4 % slower at cfg5, where
 // the ending-node rows are 64-byte neighbours in memory and concurrent quads share DRAM pages)
+template <bool kAligned>
 __device__ __forceinline__ Item decode_item(int item, int N, int H, int R) {
-    const int NRQ = R / NG, NQB = (N + BQ - 1) / BQ;
+    const int NRQ = R / NG, NQB = kAligned ? N / BQ : (N + BQ - 1) / BQ;
     Item it;
     it.r4 = (item % NRQ) * NG;
     int t = item / NRQ;
@@ -68,6 +69,8 @@ __device__ __forceinline__ Item decode_item(int item, int N, int H, int R) {
     return it;
 }
 
+// kAligned: N % 128 == 0 (no partial tile anywhere: the bounds checks fold away)
+template <bool kAligned>
 __global__ void __launch_bounds__(FWD_THREADS, 1)
 sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                  const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmBias, Problem p,
@@ -93,7 +96,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
 
     const int tid = threadIdx.x, warp = tid >> 5;
     const int N = p.N;
-    const int TPR = (N + BK - 1) / BK;  // key tiles per row (the last one may be partial: TMA zero-fills, the mask bits hide it)
+    const int TPR = kAligned ? N / BK : (N + BK - 1) / BK;  // key tiles per row (the last one may be partial: TMA zero-fills, the mask bits hide it)
     const int n_items = (total_items - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     const int NT_all = n_items * TPR;  // tiles per group over the CTA's life
 
@@ -120,7 +123,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
             // ---- TMA producer: bias tile of (item, kt) once, then (Q at kt = 0,) K, V of every group ----
             int kst = 0, kph = 0, bst = 0, bph = 0;
             for (int il = 0; il < n_items; ++il) {
-                const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
+                const Item it = decode_item<kAligned>((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
                 const int bh = it.b * p.H + it.h;
                 for (int kt = 0; kt < TPR; ++kt) {
                     mbar_wait(bias_free + bst, bph ^ 1);
@@ -200,13 +203,13 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         const uint32_t tS = tmem + g * 128 + lane_off, tP = tS + 64, tO = tS + 96;
         const float sl = rsqrtf((float)DH) * kLog2e;  // scores are kept in log2 units: x = S * scale * log2e + log2e * bias
         const uint64_t sl2 = pack2(sl, sl);
-        const int NW = (N + 63) / 64;  // mask words per row
+        const int NW = kAligned ? N / 64 : (N + 63) / 64;  // mask words per row
         int bst = 0, bph = 0;
         int n = 0;
         uint64_t* my_tok = tok + g * 4 + (warp & 3);
         uint64_t* next_tok = tok + ((g + 1) % NG) * 4 + (warp & 3);
         for (int il = 0; il < n_items; ++il) {
-            const Item it = decode_item((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
+            const Item it = decode_item<kAligned>((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
             const int r = it.r4 + g;
             const unsigned long long* mrow = maskbits ? maskbits + ((long long)it.b * p.R + r) * NW : nullptr;
             uint64_t mb_next = mrow ? ldg_u64(mrow) : ~0ull;
@@ -305,7 +308,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 warp_arrive(p_ready + g);
             }
             // ---- row epilogue: O = sigmoid(G) * O_r / l ; LSE = m + ln l -------------------------------
-            const bool inq = it.q0 + row < N;  // the last query block may be partial
+            const bool inq = kAligned || it.q0 + row < N;  // the last query block may be partial
             uint4 gv[4];
             const uint4* gp = (const uint4*)(G + off);
 #pragma unroll
@@ -457,14 +460,14 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
         !make_tmap_u(&tV, V, p.B, p.N, p.H, p.d, p.variant, BK, p.R) || !make_tmap_plane_f32(&tB, biasL, p.B * p.H, p.N, BQ))
         return cuda_fail(cudaErrorUnknown, "cuTensorMapEncodeTiled");
     // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
-    TRI_CUDA_CHECK(cudaFuncSetAttribute(sm100_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));
+    auto kern = p.N % 128 == 0 ? sm100_fwd_kernel<true> : sm100_fwd_kernel<false>;
+    TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));
     const long long items = (long long)p.B * p.H * ((p.N + BQ - 1) / BQ) * (p.R / NG);
     const int grid = (int)(items < sm_count() ? items : sm_count());
     {
         ProfScope ps("sm100_fwd_kernel", st);
-        sm100_fwd_kernel<<<grid, FWD_THREADS, FwdSmem::total, st>>>(tQ, tK, tV, tB, p, (const __nv_bfloat16*)G,
-                                                                    (const unsigned long long*)maskbits,
-                                                                    (__nv_bfloat16*)O, LSE, (int)items);
+        kern<<<grid, FWD_THREADS, FwdSmem::total, st>>>(tQ, tK, tV, tB, p, (const __nv_bfloat16*)G, (const unsigned long long*)maskbits,
+                                                        (__nv_bfloat16*)O, LSE, (int)items);
     }
     TRI_LAUNCH_CHECK("sm100_fwd_kernel");
     return TRI_OK;
