@@ -85,7 +85,8 @@ typedef enum {
     TRI_ERR_INVALID_ARG = 1, /* NULL / misaligned pointer, non-positive size, bad enum            */
     TRI_ERR_UNSUPPORTED = 2, /* shape or dtype outside the supported set                           */
     TRI_ERR_WORKSPACE = 3,   /* workspace NULL / misaligned / smaller than *_workspace_bytes()      */
-    TRI_ERR_CUDA = 4         /* a CUDA runtime / driver call or a kernel launch failed             */
+    TRI_ERR_CUDA = 4,        /* a CUDA runtime / driver call or a kernel launch failed             */
+    TRI_ERR_TOO_LARGE = 5    /* tri_attn_fwd_noalloc: the problem needs more scratch than the built-in array holds */
 } tri_status;
 
 typedef enum { TRI_F32 = 0, TRI_BF16 = 1 } tri_dtype;
@@ -133,6 +134,26 @@ TRI_API tri_status tri_attn_rows_bwd(const void* dO,
                              void* dQ, void* dK, void* dV, void* dG, float* dBias,
                              int B, int R, int N, int H, int d, tri_dtype dtype,
                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Forward WITHOUT a caller workspace and without any device allocation (for callers that cannot call cudaMalloc: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same operation, arguments, layouts and
+ * results as tri_attn_fwd (Listing 1 P:L153-185 + gate + mask); the scratch tri_attn_fwd takes from `workspace` lives in
+ * one file-scope device array of TRI_NOALLOC_SCRATCH_BYTES inside the library, which every GPU that loads the library
+ * holds until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine).
+ *   - Limit: problems with tri_attn_fwd_workspace_bytes() > TRI_NOALLOC_SCRATCH_BYTES (32 MiB; e.g. bf16 d = 32 with
+ *     B*H*N*N > ~8.3 M: cfg4 B=2 H=4 N=768 and cfg5 B=1 H=4 N=1024 fit, N = 2048 with H = 4 does not) return
+ *     TRI_ERR_TOO_LARGE before any launch; use tri_attn_fwd with a workspace for those.
+ *   - The array is shared by every call on a device and keeps the last call's contents (each call overwrites what it
+ *     reads, nothing needs clearing).  Calls that overlap on the GPU -- different streams, or host threads without
+ *     stream ordering between their calls -- RACE on it: keep the calls of one device on one stream, or order them.
+ *   - Other errors as tri_attn_fwd. */
+#define TRI_NOALLOC_SCRATCH_BYTES (32u << 20)
+TRI_API size_t tri_attn_noalloc_scratch_bytes(void);
+TRI_API tri_status tri_attn_fwd_noalloc(const void* Q, const void* K, const void* V, const void* G,
+                                const void* bias, const unsigned char* mask /* NULL = no mask */,
+                                void* O, float* LSE,
+                                int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
+                                void* cuda_stream);
 
 /* End-to-end step on HOST buffers: H2D(Q,K,V,G,bias,mask,dO) -> fwd -> bwd -> D2H(O,LSE,dQ,dK,dV,
  * dG,dBias).  `arena` is a caller-owned device buffer of tri_attn_step_host_arena_bytes() bytes. */

@@ -30,6 +30,8 @@ SIGNATURES = {
     "tri_attn_rows_bwd_workspace_bytes": (_sz, [_i] * 6),
     "tri_attn_rows_fwd": (_i, [_vp] * 8 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_rows_bwd": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
+    "tri_attn_noalloc_scratch_bytes": (_sz, []),
+    "tri_attn_fwd_noalloc": (_i, [_vp] * 8 + [_i] * 6 + [_vp]),
     "tri_attn_step_host_arena_bytes": (_sz, [_i] * 6),
     "tri_attn_step_host": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_uses_tensor_cores": (_i, [_i] * 6),
@@ -258,6 +260,34 @@ def tri_attn_rows_bwd(dO, Q, K, V, G, bias, mask, O, LSE, out=None, workspace=No
                                      _ptr(LSE), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(dG), _ptr(dBias),
                                      B, R, N, H, d, code, _ptr(ws), ws.numel(), stream))
     return dQ, dK, dV, dG, dBias
+
+
+def noalloc_scratch_bytes() -> int:
+    """Size of the library's built-in scratch array: the limit of tri_attn_fwd_noalloc."""
+    return int(load().tri_attn_noalloc_scratch_bytes())
+
+
+def tri_attn_fwd_noalloc(Q, K, V, G, bias, mask, variant, O, LSE):
+    """Forward into the caller's O, LSE with the scratch in the library's built-in device array: nothing is allocated,
+    here or in the library (every tensor, outputs included, comes from the caller).  See include/tri_attn.h for the
+    size limit and for why overlapping calls race."""
+    lib = load()
+    if not Q.is_cuda:
+        raise TriAttnError("tri_attn_fwd_noalloc needs CUDA tensors (there is no CPU path)")
+    B, N, H, d = _dims(Q)
+    dt, dev = Q.dtype, Q.device
+    for t, n in ((Q, "Q"), (K, "K"), (V, "V"), (G, "G"), (O, "O")):
+        _chk(t, Q.shape, dt, n, dev)
+    _chk(bias, (B, H, N, N), dt, "bias", dev)
+    _chk(mask, (B, N, N), torch.uint8, "mask", dev)
+    _chk(LSE, (B, N, H, N), torch.float32, "LSE", dev)
+    if O is None or LSE is None:
+        raise TriAttnError("tri_attn_fwd_noalloc: O and LSE must be preallocated by the caller")
+    with torch.cuda.device(dev):
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(lib.tri_attn_fwd_noalloc(_ptr(Q), _ptr(K), _ptr(V), _ptr(G), _ptr(bias), _ptr(mask), _ptr(O), _ptr(LSE),
+                                        B, N, H, d, variant, _dtype_code(Q), stream))
+    return O, LSE
 
 
 def step_host_arena_bytes(B, N, H, d, variant, dtype_code) -> int:

@@ -430,6 +430,7 @@ const char* tri_status_string(tri_status s) {
         case TRI_ERR_UNSUPPORTED: return "TRI_ERR_UNSUPPORTED: shape or dtype outside the supported set";
         case TRI_ERR_WORKSPACE: return "TRI_ERR_WORKSPACE: workspace null, misaligned or too small";
         case TRI_ERR_CUDA: return "TRI_ERR_CUDA: a CUDA call or kernel launch failed";
+        case TRI_ERR_TOO_LARGE: return "TRI_ERR_TOO_LARGE: the problem needs more scratch than the library's built-in array holds (tri_attn_fwd_noalloc); use the workspace entry point";
     }
     return "unknown tri_status";
 }
