@@ -468,3 +468,64 @@ def test_evosp_row_shards_reproduce_the_unsharded_kernels(tri):
             dsum += outs[6].double()
         ref = full["dBias"].double()
         assert float((dsum - ref).abs().max() / ref.abs().max()) <= 1e-5
+
+
+@pytest.mark.parametrize("variant,N,R", [(STARTING, 200, None), (ENDING, 328, None), (STARTING, 256, 100), (ENDING, 128, None)])
+def test_no_store_outside_the_output_tensors_and_workspace(tri, variant, N, R):
+    """compute-sanitizer is closed on this pool, so out-of-bounds stores are looked for directly: every output tensor and
+    the workspace sit in one allocation between 64 KB guard bands of a known byte pattern; after forward + backward (partial
+    tiles at N = 200 / 328, R != N rows, aligned N = 128) every guard byte must be untouched and every output element
+    written (the outputs start as NaN / 0xFF patterns)."""
+    import torch
+
+    B, H, d, GUARD = 2, 2, 32, 64 << 10
+    rows = N if R is None else R
+    cfg = tri_inputs.small_config(B, max(N, rows), H, d, "bf16", variant, 1.0, "none", seed=5 + N)
+    sq = tri_inputs.make_inputs(cfg)
+    if variant == STARTING:
+        x = {k: np.ascontiguousarray(sq[k][:, :rows, :, :N, :]) for k in ("Q", "K", "V", "G", "dO")}
+    else:
+        x = {k: sq[k] for k in ("Q", "K", "V", "G", "dO")}
+    x["bias"] = np.ascontiguousarray(sq["bias"][:, :, :N, :N])
+    x["mask"] = None
+    g = pu.gpu_inputs(x, "bf16")
+    U = B * rows * H * N * d
+    if R is None:
+        wsb = max(tri.fwd_workspace_bytes(B, N, H, d, variant, tri.BF16), tri.bwd_workspace_bytes(B, N, H, d, variant, tri.BF16))
+    else:
+        wsb = max(tri.rows_fwd_workspace_bytes(B, R, N, H, d, tri.BF16), tri.rows_bwd_workspace_bytes(B, R, N, H, d, tri.BF16))
+    sizes = [("O", U * 2), ("LSE", B * rows * H * N * 4), ("dQ", U * 2), ("dK", U * 2), ("dV", U * 2), ("dG", U * 2),
+             ("dBias", B * H * N * N * 4), ("ws", wsb)]
+    offs, o = {}, GUARD
+    for name, nb in sizes:
+        offs[name] = o
+        o += (nb + 255) // 256 * 256 + GUARD
+    arena = torch.full((o,), 0xA5, dtype=torch.uint8, device="cuda")
+
+    def view(name, dtype, shape):
+        nb = dict(sizes)[name]
+        t = arena[offs[name]:offs[name] + nb]
+        t.fill_(0xFF)  # bf16 0xFFFF and fp32 0xFFFFFFFF are NaNs
+        return t.view(dtype).view(shape)
+
+    shp = (B, rows, H, N, d)
+    O, dQ, dK, dV, dG = (view(n, torch.bfloat16, shp) for n in ("O", "dQ", "dK", "dV", "dG"))
+    LSE = view("LSE", torch.float32, (B, rows, H, N))
+    dBias = view("dBias", torch.float32, (B, H, N, N))
+    ws = arena[offs["ws"]:offs["ws"] + wsb]
+    if R is None:
+        tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], None, variant, O=O, LSE=LSE, workspace=ws)
+        tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], None, O, LSE, variant, out=(dQ, dK, dV, dG, dBias),
+                         workspace=ws)
+    else:
+        tri.tri_attn_rows_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], None, O=O, LSE=LSE, workspace=ws)
+        tri.tri_attn_rows_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], None, O, LSE, out=(dQ, dK, dV, dG, dBias),
+                              workspace=ws)
+    torch.cuda.synchronize()
+    for t, n in ((O, "O"), (LSE, "LSE"), (dQ, "dQ"), (dK, "dK"), (dV, "dV"), (dG, "dG"), (dBias, "dBias")):
+        assert bool(torch.isfinite(t.float()).all()), f"{n}: elements left unwritten (or non-finite)"
+    guard = torch.ones(o, dtype=torch.bool, device="cuda")
+    for name, nb in sizes:
+        guard[offs[name]:offs[name] + nb] = False
+    bad = (arena != 0xA5) & guard
+    assert not bool(bad.any()), f"guard bytes overwritten at offsets {torch.nonzero(bad)[:8].flatten().tolist()} (layout {offs})"
