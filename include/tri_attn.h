@@ -41,6 +41,9 @@
  *     least *_workspace_bytes() bytes, contents undefined on entry and exit).  workspace_bytes is
  *     O(B*H*N^2*d) (the backward keeps one dA = dO (.) sigmoid(G) tensor there); nothing of size
  *     B*H*N^3 exists anywhere.
+ *   - tri_attn_fwd / tri_attn_bwd / tri_attn_rows_* enqueue stream work only (kernels and the event fork / join of the
+ *     side streams), so a step can be captured into a CUDA graph on `cuda_stream` and replayed (tested; make one eager
+ *     call first so that the library's streams, events and tensor maps exist before the capture).
  *   - Outputs (and the workspace) must not overlap inputs or each other: such a call returns
  *     TRI_ERR_INVALID_ARG before any launch.  Outputs are overwritten (dBias is NOT accumulated into).  Results are bitwise reproducible run to run (no floating-point atomics).
  *   - tri_attn_step_host takes HOST pointers (pinned memory recommended) for every tensor plus a

@@ -529,3 +529,45 @@ def test_no_store_outside_the_output_tensors_and_workspace(tri, variant, N, R):
         guard[offs[name]:offs[name] + nb] = False
     bad = (arena != 0xA5) & guard
     assert not bool(bad.any()), f"guard bytes overwritten at offsets {torch.nonzero(bad)[:8].flatten().tolist()} (layout {offs})"
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3e"])
+def test_forward_backward_capture_into_a_cuda_graph(tri, name):
+    """tri_attn_fwd + tri_attn_bwd enqueue only stream work (kernels, event fork / join of the library's side streams), so
+    a caller can capture a step into a CUDA graph; the replay must give bitwise the eager results (and capture itself must
+    not run anything)."""
+    import torch
+
+    cfg = tri_inputs.CONFIGS[name]
+    x = tri_inputs.make_inputs(cfg)
+    _, eager = pu.run_gpu(x, cfg.dtype, cfg.variant)
+    g = pu.gpu_inputs(x, cfg.dtype)
+    B, N, H, d = cfg.B, cfg.N, cfg.H, cfg.d
+    O = torch.zeros_like(g["Q"])
+    LSE = torch.zeros((B, N, H, N), dtype=torch.float32, device="cuda")
+    grads = tuple(torch.zeros_like(g["Q"]) for _ in range(4)) + (torch.zeros((B, H, N, N), dtype=torch.float32, device="cuda"),)
+    code = tri.BF16 if cfg.dtype == "bf16" else tri.F32
+    ws = torch.empty(max(tri.fwd_workspace_bytes(B, N, H, d, cfg.variant, code), tri.bwd_workspace_bytes(B, N, H, d, cfg.variant, code)),
+                     dtype=torch.uint8, device="cuda")
+
+    def step():
+        tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], cfg.variant, O=O, LSE=LSE, workspace=ws)
+        tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], O, LSE, cfg.variant, out=grads, workspace=ws)
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        step()  # first use of the library's streams / tensor maps happens outside the capture
+    torch.cuda.synchronize()
+    for t in (O, LSE) + grads:
+        t.zero_()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        step()
+    torch.cuda.synchronize()
+    assert float(O.float().abs().sum()) == 0.0  # nothing ran during capture
+    for _ in range(2):
+        graph.replay()
+    torch.cuda.synchronize()
+    for k, t in zip(pu.OUT_NAMES, (O, LSE) + grads):
+        assert torch.equal(t.view(torch.uint8), eager[k].view(torch.uint8)), k
