@@ -429,6 +429,13 @@ bool sm100_supported(const Problem& p, tri_dtype dt) {
            (p.R == p.N || p.variant == TRI_STARTING);
 }
 
+// The forward alone has no cluster in it: its key loop is as long as N wants (long-sequence inference).  16384 keeps
+// every item count and TMA coordinate far inside 31 bits.
+bool sm100_fwd_supported(const Problem& p, tri_dtype dt) {
+    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 16384 && p.R % 4 == 0 &&
+           (p.R == p.N || p.variant == TRI_STARTING);
+}
+
 // the kernels need the packed mask words when the caller passed a mask or when the last 64-key tile is partial
 bool sm100_needs_maskbits(const Problem& p, const unsigned char* mask) { return mask != nullptr || p.N % 64 != 0; }
 

@@ -79,7 +79,7 @@ extern "C" {
 size_t tri_attn_fwd_workspace_bytes(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype) {
     if (!shape_ok(B, N, H, d) || !enums_ok(variant, dtype) || !d_ok(d) || !size_ok(B, N, H, d)) return 0;
     Problem p = make_problem(B, N, H, d, variant);
-    size_t w = sm100_supported(p, dtype) ? sm100_fwd_workspace(p) : simt_fwd_workspace(p);
+    size_t w = sm100_fwd_supported(p, dtype) ? sm100_fwd_workspace(p) : simt_fwd_workspace(p);
     return w < 256 ? 256 : w;
 }
 
@@ -109,7 +109,7 @@ tri_status tri_attn_fwd(const void* Q, const void* K, const void* V, const void*
     }
     Problem p = make_problem(B, N, H, d, variant);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (sm100_supported(p, dtype)) return sm100_fwd(p, Q, K, V, G, bias, mask, O, LSE, workspace, st);
+    if (sm100_fwd_supported(p, dtype)) return sm100_fwd(p, Q, K, V, G, bias, mask, O, LSE, workspace, st);
     return simt_fwd(p, dtype, Q, K, V, G, bias, mask, O, LSE, workspace, st);
 }
 
@@ -142,13 +142,14 @@ tri_status tri_attn_bwd(const void* dO, const void* Q, const void* K, const void
 }
 
 // ---- decoupled row count (starting node): R broadcast rows that attend over N positions with one [B,H,N,N] bias ----
-static bool rows_ok(int B, int R, int N, int H, int d, tri_dtype dtype) {
+static bool rows_ok(int B, int R, int N, int H, int d, tri_dtype dtype, bool fwd_only = false) {
     if (!shape_ok(B, N, H, d) || R <= 0 || !d_ok(d) || !size_ok(B, R > N ? R : N, H, d)) return false;
-    return sm100_supported(make_problem(B, N, H, d, TRI_STARTING, R), dtype);
+    const Problem p = make_problem(B, N, H, d, TRI_STARTING, R);
+    return fwd_only ? sm100_fwd_supported(p, dtype) : sm100_supported(p, dtype);
 }
 
 size_t tri_attn_rows_fwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype) {
-    if (!rows_ok(B, R, N, H, d, dtype)) return 0;
+    if (!rows_ok(B, R, N, H, d, dtype, true)) return 0;
     const size_t w = sm100_fwd_workspace(make_problem(B, N, H, d, TRI_STARTING, R));
     return w < 256 ? 256 : w;
 }
@@ -165,7 +166,7 @@ tri_status tri_attn_rows_fwd(const void* Q, const void* K, const void* V, const 
     if (!shape_ok(B, N, H, d) || R <= 0 || !enums_ok(TRI_STARTING, dtype)) return TRI_ERR_INVALID_ARG;
     if (!Q || !K || !V || !G || !bias || !O || !LSE) return TRI_ERR_INVALID_ARG;
     if (!al16(Q) || !al16(K) || !al16(V) || !al16(G) || !al16(bias) || !al16(O) || !al16(LSE)) return TRI_ERR_INVALID_ARG;
-    if (!rows_ok(B, R, N, H, d, dtype)) return TRI_ERR_UNSUPPORTED;
+    if (!rows_ok(B, R, N, H, d, dtype, true)) return TRI_ERR_UNSUPPORTED;
     const size_t need = tri_attn_rows_fwd_workspace_bytes(B, R, N, H, d, dtype);
     if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < need) return TRI_ERR_WORKSPACE;
     {

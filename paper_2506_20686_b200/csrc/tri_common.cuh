@@ -90,7 +90,8 @@ tri_status simt_bwd(const Problem& p, tri_dtype dt, const void* dO, const void* 
                     float* dBias, void* ws, cudaStream_t st);
 
 // ---- bf16 tcgen05 / TMA path (sm100_fwd.cu, sm100_bwd.cu) ------------------------------------
-bool sm100_supported(const Problem& p, tri_dtype dt);
+bool sm100_supported(const Problem& p, tri_dtype dt);      // forward + backward on the tensor-core kernels
+bool sm100_fwd_supported(const Problem& p, tri_dtype dt);  // forward only (a superset: N up to 16384)
 tri_status sm100_transpose_planes(const void* in, void* out, int BH, int N, cudaStream_t st);  // bf16 [BH,N,N]
 // fp32 planes f*bias: nat (same orientation) and / or tr (transposed); either may be null
 tri_status sm100_bias_planes(const void* in, float* nat, float* tr, int BH, int N, float f, cudaStream_t st);

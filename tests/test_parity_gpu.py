@@ -571,3 +571,46 @@ def test_forward_backward_capture_into_a_cuda_graph(tri, name):
     torch.cuda.synchronize()
     for k, t in zip(pu.OUT_NAMES, (O, LSE) + grads):
         assert torch.equal(t.view(torch.uint8), eager[k].view(torch.uint8)), k
+
+
+def test_forward_beyond_n2048_stays_on_the_tensor_core_kernels(tri, oracle):
+    """Long-sequence inference: the forward has no cluster in it, so it runs on the tcgen05 kernels up to N = 16384
+    (the backward's fused dQ + dBias stage stops at 2048).  (1) rows entry point, R = 8 rows over N = 4104 positions
+    (65 key tiles, the last one partial), masked, every element of O and LSE against the oracle; (2) square ending-node
+    problem at N = 2176, H = 1: sampled rows against the oracle; the launch count shows which kernels ran."""
+    import torch
+
+    B, R, N, H, d = 1, 8, 4104, 2, 32
+    rng = np.random.default_rng(4104)
+    x = {k: tri_inputs.round_bf16(rng.standard_normal((B, R, H, N, d)).astype(np.float32)) for k in ("Q", "K", "V", "G")}
+    x["bias"] = tri_inputs.round_bf16((1.5 * rng.standard_normal((B, H, N, N))).astype(np.float32))
+    m = np.ones((B, R, N), np.uint8)
+    m[0, 1, N - 700:] = 0
+    m[0, 2, :2048 + 64] = 0
+    m[0, 3] = rng.random(N) < 0.7
+    m[0, 5, :] = 0
+    assert tri.rows_fwd_workspace_bytes(B, R, N, H, d, tri.BF16) > 0 and tri.rows_bwd_workspace_bytes(B, R, N, H, d, tri.BF16) == 0
+    g = {k: pu.to_torch(v, "bf16") for k, v in x.items()}
+    O, LSE = tri.tri_attn_rows_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], pu.to_torch(m, "u8"))
+    torch.cuda.synchronize()
+    rO, rLSE = oracle.fwd_start_general(x["Q"], x["K"], x["V"], x["G"], x["bias"], m)
+    errs = pu.assert_close({"O": O.float().cpu().numpy(), "LSE": LSE.cpu().numpy()}, {"O": rO, "LSE": rLSE}, pu.TOL["bf16"],
+                           names=("O", "LSE"), what="rows fwd N=4104")
+    print("fwd N=4104", errs)
+    assert np.isneginf(LSE.cpu().numpy()[0, 5]).all()
+
+    cfg = tri_inputs.small_config(1, 2176, 1, 32, "bf16", ENDING, 1.0, "tail:90", seed=2176)
+    xe = tri_inputs.make_inputs(cfg)
+    ge = pu.gpu_inputs(xe, "bf16")
+    assert not tri.uses_tensor_cores(1, 2176, 1, 32, ENDING, tri.BF16)  # the backward would not
+    n0 = tri.launch_count()
+    Oe, LSEe = tri.tri_attn_fwd(ge["Q"], ge["K"], ge["V"], ge["G"], ge["bias"], ge["mask"], ENDING)
+    torch.cuda.synchronize()
+    assert tri.launch_count() - n0 == 3  # pack_mask, bias_planes, sm100_fwd_kernel
+    xs = pu.to_starting(xe, ENDING)
+    gs = pu.outputs_to_starting({"O": Oe.float().cpu().numpy().astype(np.float64), "LSE": LSEe.cpu().numpy().astype(np.float64)}, ENDING)
+    rows = np.array([0, 777, 2175])
+    refO, refL = oracle.fwd_start_general(xs["Q"][:, rows], xs["K"][:, rows], xs["V"][:, rows], xs["G"][:, rows], xs["bias"],
+                                          None if xs["mask"] is None else xs["mask"][:, rows])
+    pu.assert_close({"O": gs["O"][:, rows], "LSE": gs["LSE"][:, rows]}, {"O": refO, "LSE": refL}, pu.TOL["bf16"], names=("O", "LSE"),
+                    what="fwd N=2176 ending")
