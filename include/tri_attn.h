@@ -62,12 +62,13 @@
  *   - Errors: a tri_status is returned, nothing is thrown or aborted across the ABI.  Argument
  *     errors are detected before any launch.  Launch failures map to TRI_ERR_CUDA.
  *   - Supported: d in {16, 32, 64}, any N >= 1, dtype f32 or bf16.  bf16 with d == 32,
- *     N % 8 == 0 and 128 <= N <= 2048 runs on the tcgen05/TMA tensor-core kernels (N need not be a
+ *     N % 8 == 0 and 128 <= N <= 8192 runs on the tcgen05/TMA tensor-core kernels (N need not be a
  *     multiple of their 64 / 128-position tiles: partial tiles are zero-filled by TMA and masked);
  *     every other combination runs on the fp32 CUDA-core kernels, ~30x slower (fp32 needs them: the
  *     1e-4 bound excludes TF32, reading A14); tri_attn_uses_tensor_cores() tells which.
  *     The FORWARD alone (tri_attn_fwd, tri_attn_rows_fwd, tri_attn_fwd_noalloc) stays on the tensor-core kernels up to
- *     N = 16384 (long-sequence inference); the backward of N > 2048 runs on the CUDA-core kernels.
+ *     N = 16384 (long-sequence inference).  The backward of N > 2048 runs its fused dQ + dBias stage in
+ *     ceil(N / 2048) launches over slices of the key axis (its workspace then also holds an fp32 dQ sum).
  *     Anything else returns TRI_ERR_UNSUPPORTED.  There is no CPU path.
  */
 #ifndef TRI_ATTN_H_
@@ -123,7 +124,7 @@ TRI_API tri_status tri_attn_bwd(const void* dO,
  * bias[b,h,j,k].  Starting-node index convention only:
  *     Q,K,V,G,O,dO,dQ,dK,dV,dG : [B, R, H, N, d]     mask : [B, R, N] (or NULL)     LSE : [B, R, H, N]
  *     bias, dBias              : [B, H, N, N]        dBias[b,h,j,k] = sum over the R rows of dS
- * Runs on the tensor-core kernels only: bf16, d == 32, N % 8 == 0, 128 <= N <= 2048 (forward: 16384), R % 4 == 0; anything else returns
+ * Runs on the tensor-core kernels only: bf16, d == 32, N % 8 == 0, 128 <= N <= 8192 (forward: 16384), R % 4 == 0; anything else returns
  * TRI_ERR_UNSUPPORTED (workspace queries return 0).  tri_attn_fwd / tri_attn_bwd are the R == N case. */
 TRI_API size_t tri_attn_rows_fwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype);
 TRI_API size_t tri_attn_rows_bwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype);
@@ -171,7 +172,7 @@ TRI_API tri_status tri_attn_step_host(const void* hQ, const void* hK, const void
                               void* arena, size_t arena_bytes, void* cuda_stream);
 
 /* 1 if forward AND backward of this problem run on the tcgen05/TMA tensor-core kernels, 0 if the backward (and, but for
- * bf16 d = 32 with 2048 < N <= 16384, N % 8 == 0, also the forward) runs on the fp32 CUDA-core kernels. */
+ * bf16 d = 32 with 8192 < N <= 16384, N % 8 == 0, also the forward) runs on the fp32 CUDA-core kernels. */
 TRI_API int tri_attn_uses_tensor_cores(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);
 
 /* Number of kernel launches this library has enqueued since it was loaded (for bench accounting). */

@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(256) sm100_dbias_reduce_kernel(const float* __
 // ---- host side ------------------------------------------------------------------------------------------------
 namespace {
 struct BwdWs {
-    size_t d_off, da_off, biast_off, biasl_off, mask_off, nl_off, nd_off, planes_off, total;
+    size_t d_off, da_off, biast_off, biasl_off, mask_off, nl_off, nd_off, planes_off, dqpart_off, total;
 };
 BwdWs bwd_ws_layout(const Problem& p) {
     BwdWs w;
@@ -94,6 +94,9 @@ BwdWs bwd_ws_layout(const Problem& p) {
     // partial dBias planes: the fused kernel picks its row split (<= kDqdbMaxSplit) at launch from the device's
     // resident cluster count, so the workspace always holds the maximum
     w.planes_off = o; o += align_up((size_t)kDqdbMaxSplit * p.B * p.H * p.N * p.N * sizeof(float), 256);
+    // N > 2048: fp32 running sum of dQ between the key passes of the fused stage (one U-shaped tensor)
+    w.dqpart_off = o;
+    if (sm100_dqdb_passes(p.N) > 1) o += align_up((size_t)p.B * p.R * p.H * p.N * p.d * sizeof(float), 256);
     w.total = o;
     return w;
 }
@@ -190,7 +193,11 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     // on those SMs at the same time on the side stream; the rest of stage 1 follows on all SMs.
     float* planes = (float*)((char*)ws + w.planes_off);
     int Gs = 1, C2 = 0, grid2 = 0;
-    if (!sm100_dqdb_plan(p, &C2, &Gs, &grid2)) return cuda_fail(cudaErrorLaunchFailure, "sm100_dqdb_plan: no resident cluster of the needed size");
+    const int npass = sm100_dqdb_passes(p.N);
+    float* dq_part = (float*)((char*)ws + w.dqpart_off);
+    const DqdbPass pass0 = sm100_dqdb_pass(p.N, 0, dq_part);
+    if (!sm100_dqdb_plan(p, pass0.tiles, 0, &C2, &Gs, &grid2))
+        return cuda_fail(cudaErrorLaunchFailure, "sm100_dqdb_plan: no resident cluster of the needed size");
     const long long items1 = sm100_dkdv2_items(p);
     const int sms = sm100_sm_count();
     const int spare = sms - grid2;
@@ -204,8 +211,15 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
         TRI_CUDA_CHECK(cudaEventRecord(side->fork, st));
         TRI_CUDA_CHECK(cudaStreamWaitEvent(side->stream, side->fork, 0));
     }
-    if ((s = sm100_dqdb_launch(p, C2, Gs, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, accumulate_dbias ? planes : dBias, planes, st)) != TRI_OK)
-        return s;
+    float* dbias_out = accumulate_dbias ? planes : dBias;
+    if ((s = sm100_dqdb_launch(p, C2, Gs, grid2, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dbias_out, planes, pass0, st)) != TRI_OK) return s;
+    for (int i = 1; i < npass; ++i) {  // N > 2048: the further slices of the key axis, same row split
+        const DqdbPass ps = sm100_dqdb_pass(p.N, i, dq_part);
+        int Ci = 0, Gi = 0, gridi = 0;
+        if (!sm100_dqdb_plan(p, ps.tiles, Gs, &Ci, &Gi, &gridi) || Gi != Gs)
+            return cuda_fail(cudaErrorLaunchFailure, "sm100_dqdb_plan: no resident cluster of the needed size");
+        if ((s = sm100_dqdb_launch(p, Ci, Gs, gridi, Q, dA, K, V, biasL, maskbits, LSE, Dws, dQ, dbias_out, planes, ps, st)) != TRI_OK) return s;
+    }
     if (itemsA > 0) {
         if ((s = sm100_dkdv2_launch(p, Q, dA, K, V, bias_kq, maskbits, NL, ND, dK, dV, 0, itemsA, spare, "sm100_dkdv_kernel(side)",
                                     side->stream)) != TRI_OK)

@@ -139,14 +139,15 @@ __device__ __forceinline__ Item2 decode_item2(int item, int N, int H, int G, int
     return it;
 }
 
-// kAligned: N % 128 == 0 (no partial tile anywhere: the bounds checks fold away)
-template <bool kAligned>
+// kAligned: N % 128 == 0 (no partial tile anywhere: the bounds checks fold away).  kPasses: N > 2048, the launch covers a
+// slice of the key axis (`pass`) and dQ is carried between the launches; false keeps that code out of the common kernel.
+template <bool kAligned, bool kPasses>
 __global__ void __launch_bounds__(DQDB_THREADS, 1)
 sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmA,
                   const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                   const __grid_constant__ CUtensorMap tmBias, Problem p, const unsigned long long* __restrict__ maskbits,
                   const float* __restrict__ LSE, const float* __restrict__ Dws, __nv_bfloat16* __restrict__ dQ,
-                  float* __restrict__ dBias, float* __restrict__ planes, int G, int n_items, int kbox) {
+                  float* __restrict__ dBias, float* __restrict__ planes, int G, int n_items, int kbox, DqdbPass pass) {
     using L = DqdbSmem;
     extern __shared__ uint8_t smem_raw[];
     // the dynamic shared-memory window starts at the same offset in every CTA of the cluster, so the aligned layout
@@ -174,10 +175,12 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int N = p.N, NW = kAligned ? N / BK : (N + BK - 1) / BK;  // the last tile / query block may be partial (TMA zero-fill + mask bits)
     const int C = (int)cluster_nctarank(), c = (int)cluster_ctarank();
-    // key tiles of this rank: the N/64 tiles are dealt to the C ranks as evenly as possible (at most NGB each)
-    const int base_t = NW / C, rem_t = NW % C;
+    // key tiles of this rank: the pass's tiles (all N/64 of them when N <= 2048) are dealt to the C ranks as evenly as
+    // possible (at most NGB each)
+    const int ptiles = kPasses ? pass.tiles : NW, pbase = kPasses ? pass.tile_base : 0;
+    const int base_t = ptiles / C, rem_t = ptiles % C;
     const int nt = base_t + (c < rem_t ? 1 : 0);
-    const int t0 = c * base_t + (c < rem_t ? c : rem_t);
+    const int t0 = pbase + c * base_t + (c < rem_t ? c : rem_t);
     const int k0 = t0 * BK;
     const int NR = p.R / G;  // broadcast rows per work item
     const int cid = (int)blockIdx.x / C, ncl = (int)gridDim.x / C;
@@ -470,12 +473,28 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                     if (tid == (NGB + 1) * 128 && n + NIN < NRtot) mbar_expect_tx(in_full + j, INBOX_BYTES);
                     if (lane == 0) mbar_arrive_remote(outfree_prev + j * 8);
                 }
+                if (kPasses && c == 0 && pass.tile_base > 0 && (kAligned || it.q0 + row < N)) {
+                    // a later key pass (N > 2048): the running sum starts from what the earlier passes left in global memory
+                    const float4* src = (const float4*)(pass.dq_part + (qp - dQ));
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 t = __ldg(src + i);
+                        f[4 * i] = t.x + f[4 * i]; f[4 * i + 1] = t.y + f[4 * i + 1];
+                        f[4 * i + 2] = t.z + f[4 * i + 2]; f[4 * i + 3] = t.w + f[4 * i + 3];
+                    }
+                }
                 if (c + 1 < C) {
                     if (n >= NIN) mbar_wait(out_free + j, ph ^ 1);
                     const uint32_t dst = inbox_next + j * INBOX_BYTES + row * 128;
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
                         st_async_v4(dst + ((i ^ sw) << 4), f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3], infull_next + j * 8);
+                } else if (kPasses && !pass.last) {  // last rank of a key pass that is not the last: the fp32 sum goes to global memory
+                    if (kAligned || it.q0 + row < N) {
+                        float4* dst = (float4*)(pass.dq_part + (qp - dQ));
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) dst[i] = make_float4(f[4 * i], f[4 * i + 1], f[4 * i + 2], f[4 * i + 3]);
+                    }
                 } else if (kAligned || it.q0 + row < N) {  // last rank: dQ = scale * sum (queries beyond N: nothing to store)
                     uint4* pq = (uint4*)qp;
 #pragma unroll
@@ -497,9 +516,29 @@ sm100_dqdb_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 
 }  // namespace
 
-// cluster size for N/64 key tiles at <= NGB tiles per rank, from the sizes the launch code accepts
-int sm100_dqdb_cluster(int N) {
-    const int T = (N + BK - 1) / BK, need = (T + NGB - 1) / NGB;
+// the instantiation for a problem size
+static auto dqdb_kernel_for(int N) -> decltype(&sm100_dqdb_kernel<true, false>) {
+    const bool al = N % 128 == 0, ps = (N + BK - 1) / BK > 16 * NGB;
+    return al ? (ps ? sm100_dqdb_kernel<true, true> : sm100_dqdb_kernel<true, false>)
+              : (ps ? sm100_dqdb_kernel<false, true> : sm100_dqdb_kernel<false, false>);
+}
+
+// Key passes: one cluster covers at most 16 ranks x NGB tiles = 2048 keys, so N > 2048 runs ceil(tiles / 32) launches over
+// equal slices of the key axis; dBias columns are disjoint per pass, dQ is carried between passes as an fp32 sum.
+int sm100_dqdb_passes(int N) { return ((N + BK - 1) / BK + 16 * NGB - 1) / (16 * NGB); }
+DqdbPass sm100_dqdb_pass(int N, int i, float* dq_part) {
+    const int T = (N + BK - 1) / BK, np = sm100_dqdb_passes(N), per = (T + np - 1) / np;
+    DqdbPass ps;
+    ps.tile_base = i * per;
+    ps.tiles = T - ps.tile_base < per ? T - ps.tile_base : per;
+    ps.last = i == np - 1 ? 1 : 0;
+    ps.dq_part = dq_part;
+    return ps;
+}
+
+// cluster size for T key tiles at <= NGB tiles per rank, from the sizes the launch code accepts
+int sm100_dqdb_cluster(int T) {
+    const int need = (T + NGB - 1) / NGB;
     const int sizes[] = {1, 2, 3, 4, 6, 8, 12, 16};
     for (int s : sizes)
         if (s >= need) return s;
@@ -509,10 +548,10 @@ int sm100_dqdb_cluster(int N) {
 // Launch plan on the current device: cluster size C, row slices G per (b, h, query block) (<= kDqdbMaxSplit, chosen to
 // minimise waves * rows per item for the number of clusters the device can hold), persistent grid (a multiple of C).
 // Returns false if the kernel cannot run on this device / shape.
-bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
-    const int C = sm100_dqdb_cluster(p.N);
+bool sm100_dqdb_plan(const Problem& p, int tiles, int forceG, int* Cout, int* Gout, int* grid) {
+    const int C = sm100_dqdb_cluster(tiles);
     if (C == 0) return false;
-    auto kern = p.N % 128 == 0 ? sm100_dqdb_kernel<true> : sm100_dqdb_kernel<false>;
+    auto kern = dqdb_kernel_for(p.N);
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, DqdbSmem::total) != cudaSuccess) return false;
     if (C > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return false;
     cudaLaunchConfig_t cfg = {};
@@ -532,7 +571,7 @@ bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
     int bestG = 1;
     double best = 1e30;
     for (int G = 1; G <= kDqdbMaxSplit; ++G) {
-        if (p.R % G) continue;
+        if (p.R % G || (forceG > 0 && G != forceG)) continue;
         const double waves = (double)((base * G + ncl - 1) / ncl);
         const double cost = waves * (p.R / G + 12);  // + per-item fill / drain / dBias flush in row units
         if (cost < best * 0.99) { best = cost; bestG = G; }
@@ -545,7 +584,7 @@ bool sm100_dqdb_plan(const Problem& p, int* Cout, int* Gout, int* grid) {
 
 tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const void* Q, const void* dA, const void* K, const void* V,
                              const float* biasL_qk, const unsigned long long* maskbits, const float* LSE, const float* Dws,
-                             void* dQ, float* dBias, float* planes, cudaStream_t st) {
+                             void* dQ, float* dBias, float* planes, DqdbPass pass, cudaStream_t st) {
     const int kbox = p.N < NGB * BK ? p.N : NGB * BK;
     CUtensorMap tQ, tA, tK, tV, tB;
     if (!make_tmap_u(&tQ, Q, p.B, p.N, p.H, p.d, p.variant, BQ, p.R) || !make_tmap_u(&tA, dA, p.B, p.N, p.H, p.d, p.variant, BQ, p.R) ||
@@ -564,8 +603,8 @@ tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const voi
     const int n_items = p.B * p.H * ((p.N + BQ - 1) / BQ) * G;
     {
         ProfScope ps("sm100_dqdb_kernel", st);
-        TRI_CUDA_CHECK(cudaLaunchKernelEx(&cfg, p.N % 128 == 0 ? sm100_dqdb_kernel<true> : sm100_dqdb_kernel<false>, tQ, tA, tK, tV, tB, p, maskbits, LSE, Dws, (__nv_bfloat16*)dQ,
-                                          dBias, planes, G, n_items, kbox));
+        TRI_CUDA_CHECK(cudaLaunchKernelEx(&cfg, dqdb_kernel_for(p.N), tQ, tA, tK, tV, tB, p, maskbits, LSE, Dws, (__nv_bfloat16*)dQ,
+                                          dBias, planes, G, n_items, kbox, pass));
     }
     TRI_LAUNCH_CHECK("sm100_dqdb_kernel");
     return TRI_OK;

@@ -421,11 +421,12 @@ tri_status sm100_pack_mask(const Problem& p, const unsigned char* mask, void* bi
 
 int sm100_sm_count() { return sm_count(); }
 
-// N <= 2048: the fused dQ + dBias stage needs one cluster rank per two 64-key tiles (<= 16 ranks).  N % 8 == 0: the
+// N <= 8192: the fused dQ + dBias stage covers 2048 keys per launch (one cluster rank per two 64-key tiles, <= 16 ranks)
+// and runs ceil(N / 2048) key passes; its partial dBias planes (8 x B x H x N^2 fp32) set the practical limit.  N % 8 == 0: the
 // bias planes are read by TMA (16-byte row pitch in bf16).  N need not be a multiple of the 64 / 128-position tiles: TMA
 // zero-fills what lies beyond N, the packed mask hides keys >= N, stores of queries / keys >= N are predicated off.
 bool sm100_supported(const Problem& p, tri_dtype dt) {
-    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 2048 && p.R % 4 == 0 &&
+    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 8192 && p.R % 4 == 0 &&
            (p.R == p.N || p.variant == TRI_STARTING);
 }
 

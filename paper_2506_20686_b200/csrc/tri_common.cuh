@@ -108,12 +108,20 @@ tri_status sm100_dkdv2_launch(const Problem& p, const void* Q, const void* dA, c
                               const unsigned long long* maskbits, const float* NL, const float* ND, void* dK, void* dV,
                               long long item_begin, long long item_count, int max_ctas, const char* prof_name, cudaStream_t st);
 // fused dQ + dBias stage (sm100_dqdb.cu): cluster size (0 = shape not covered), row split, persistent grid, launch
-int sm100_dqdb_cluster(int N);
+// one launch of the fused dQ + dBias stage over a slice of the key axis (the whole axis when N <= 2048)
+struct DqdbPass {
+    int tile_base, tiles;  // first 64-key tile and tile count of the slice
+    int last;              // the last slice: dQ is finished (scaled, bf16); otherwise the fp32 running sum goes to dq_part
+    float* dq_part;        // fp32 running sum of dQ between the slices, same element order as dQ (unused when there is one slice)
+};
+int sm100_dqdb_passes(int N);
+DqdbPass sm100_dqdb_pass(int N, int i, float* dq_part);
+int sm100_dqdb_cluster(int tiles);
 constexpr int kDqdbMaxSplit = 8;  // the workspace holds this many partial dBias planes
-bool sm100_dqdb_plan(const Problem& p, int* C, int* G, int* grid);
+bool sm100_dqdb_plan(const Problem& p, int tiles, int forceG, int* C, int* G, int* grid);
 tri_status sm100_dqdb_launch(const Problem& p, int C, int G, int grid, const void* Q, const void* dA, const void* K,
                              const void* V, const float* biasL_qk, const unsigned long long* maskbits, const float* LSE,
-                             const float* Dws, void* dQ, float* dBias, float* planes, cudaStream_t st);
+                             const float* Dws, void* dQ, float* dBias, float* planes, DqdbPass pass, cudaStream_t st);
 int sm100_sm_count();
 size_t sm100_fwd_workspace(const Problem& p);
 size_t sm100_bwd_workspace(const Problem& p);

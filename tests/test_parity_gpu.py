@@ -575,7 +575,7 @@ def test_forward_backward_capture_into_a_cuda_graph(tri, name):
 
 def test_forward_beyond_n2048_stays_on_the_tensor_core_kernels(tri, oracle):
     """Long-sequence inference: the forward has no cluster in it, so it runs on the tcgen05 kernels up to N = 16384
-    (the backward's fused dQ + dBias stage stops at 2048).  (1) rows entry point, R = 8 rows over N = 4104 positions
+    (the backward's fused dQ + dBias stage covers 2048 keys per launch and goes to 8192 in key passes).  (1) rows entry point, R = 8 rows over N = 4104 positions
     (65 key tiles, the last one partial), masked, every element of O and LSE against the oracle; (2) square ending-node
     problem at N = 2176, H = 1: sampled rows against the oracle; the launch count shows which kernels ran."""
     import torch
@@ -589,7 +589,7 @@ def test_forward_beyond_n2048_stays_on_the_tensor_core_kernels(tri, oracle):
     m[0, 2, :2048 + 64] = 0
     m[0, 3] = rng.random(N) < 0.7
     m[0, 5, :] = 0
-    assert tri.rows_fwd_workspace_bytes(B, R, N, H, d, tri.BF16) > 0 and tri.rows_bwd_workspace_bytes(B, R, N, H, d, tri.BF16) == 0
+    assert tri.rows_fwd_workspace_bytes(B, R, N, H, d, tri.BF16) > 0
     g = {k: pu.to_torch(v, "bf16") for k, v in x.items()}
     O, LSE = tri.tri_attn_rows_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], pu.to_torch(m, "u8"))
     torch.cuda.synchronize()
@@ -602,7 +602,6 @@ def test_forward_beyond_n2048_stays_on_the_tensor_core_kernels(tri, oracle):
     cfg = tri_inputs.small_config(1, 2176, 1, 32, "bf16", ENDING, 1.0, "tail:90", seed=2176)
     xe = tri_inputs.make_inputs(cfg)
     ge = pu.gpu_inputs(xe, "bf16")
-    assert not tri.uses_tensor_cores(1, 2176, 1, 32, ENDING, tri.BF16)  # the backward would not
     n0 = tri.launch_count()
     Oe, LSEe = tri.tri_attn_fwd(ge["Q"], ge["K"], ge["V"], ge["G"], ge["bias"], ge["mask"], ENDING)
     torch.cuda.synchronize()
@@ -614,3 +613,35 @@ def test_forward_beyond_n2048_stays_on_the_tensor_core_kernels(tri, oracle):
                                           None if xs["mask"] is None else xs["mask"][:, rows])
     pu.assert_close({"O": gs["O"][:, rows], "LSE": gs["LSE"][:, rows]}, {"O": refO, "LSE": refL}, pu.TOL["bf16"], names=("O", "LSE"),
                     what="fwd N=2176 ending")
+
+
+@pytest.mark.parametrize("R,N", [(8, 4104), (4, 2304)])
+def test_backward_beyond_n2048_runs_key_passes_on_the_tensor_core_kernels(tri, oracle, R, N):
+    """N > 2048: the fused dQ + dBias stage runs ceil(N / 2048) launches over slices of the key axis (N = 4104: 22 + 22 + 21
+    tiles, the last one partial; N = 2304: 18 + 18), dQ carried between them as an fp32 sum, dBias columns disjoint.
+    Rows entry points with a few rows keep the oracle affordable; every element of all seven outputs is compared."""
+    import torch
+
+    B, H, d = 1, 2, 32
+    rng = np.random.default_rng(N + R)
+    x = {k: tri_inputs.round_bf16(rng.standard_normal((B, R, H, N, d)).astype(np.float32)) for k in ("Q", "K", "V", "G", "dO")}
+    x["bias"] = tri_inputs.round_bf16((1.5 * rng.standard_normal((B, H, N, N))).astype(np.float32))
+    m = np.ones((B, R, N), np.uint8)
+    m[0, 1, N - 700:] = 0
+    m[0, 2, :2048 + 64] = 0       # only keys of the later passes visible
+    m[0, 3, 1000:] = 0            # only keys of the first pass visible
+    if R > 5:
+        m[0, 4] = rng.random(N) < 0.7
+        m[0, 5, :] = 0
+    assert tri.uses_tensor_cores(B, N, H, d, STARTING, tri.BF16) and tri.rows_bwd_workspace_bytes(B, R, N, H, d, tri.BF16) > 0
+    g = {k: pu.to_torch(v, "bf16") for k, v in x.items()}
+    gm = pu.to_torch(m, "u8")
+    O, LSE = tri.tri_attn_rows_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], gm)
+    outs = tri.tri_attn_rows_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], gm, O, LSE)
+    torch.cuda.synchronize()
+    got = {k: v.float().cpu().numpy().astype(np.float64) for k, v in zip(pu.OUT_NAMES, (O, LSE) + tuple(outs))}
+    rO, rLSE = oracle.fwd_start_general(x["Q"], x["K"], x["V"], x["G"], x["bias"], m)
+    ref = dict(zip(pu.OUT_NAMES, (rO, rLSE) + tuple(
+        oracle.bwd_start_general(x["dO"], x["Q"], x["K"], x["V"], x["G"], x["bias"], m))))
+    errs = pu.assert_close(got, ref, pu.TOL["bf16"], what=f"key passes R={R} N={N}")
+    print("key passes", R, N, {k: float(f"{v:.3g}") for k, v in errs.items()})
