@@ -124,7 +124,7 @@ TRI_API tri_status tri_attn_bwd(const void* dO,
  * bias[b,h,j,k].  Starting-node index convention only:
  *     Q,K,V,G,O,dO,dQ,dK,dV,dG : [B, R, H, N, d]     mask : [B, R, N] (or NULL)     LSE : [B, R, H, N]
  *     bias, dBias              : [B, H, N, N]        dBias[b,h,j,k] = sum over the R rows of dS
- * Runs on the tensor-core kernels only: bf16, d == 32, N % 8 == 0, 128 <= N <= 8192 (forward: 16384), R % 4 == 0; anything else returns
+ * Runs on the tensor-core kernels only: bf16, d == 32, N % 8 == 0, 128 <= N <= 8192 (forward: 16384), any R >= 1 (R = 1 is single-representation attention with pair bias); anything else returns
  * TRI_ERR_UNSUPPORTED (workspace queries return 0).  tri_attn_fwd / tri_attn_bwd are the R == N case. */
 TRI_API size_t tri_attn_rows_fwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype);
 TRI_API size_t tri_attn_rows_bwd_workspace_bytes(int B, int R, int N, int H, int d, tri_dtype dtype);

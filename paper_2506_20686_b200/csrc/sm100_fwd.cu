@@ -58,7 +58,7 @@ struct Item { int b, h, q0, r4; };
 // the ending-node rows are 64-byte neighbours in memory and concurrent quads share DRAM pages)
 template <bool kAligned>
 __device__ __forceinline__ Item decode_item(int item, int N, int H, int R) {
-    const int NRQ = R / NG, NQB = kAligned ? N / BQ : (N + BQ - 1) / BQ;
+    const int NRQ = (R + NG - 1) / NG, NQB = kAligned ? N / BQ : (N + BQ - 1) / BQ;  // the last row quad may be partial
     Item it;
     it.r4 = (item % NRQ) * NG;
     int t = item / NRQ;
@@ -211,7 +211,8 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
         for (int il = 0; il < n_items; ++il) {
             const Item it = decode_item<kAligned>((int)blockIdx.x + il * (int)gridDim.x, N, p.H, p.R);
             const int r = it.r4 + g;
-            const unsigned long long* mrow = maskbits ? maskbits + ((long long)it.b * p.R + r) * NW : nullptr;
+            const bool rin = r < p.R;  // a group beyond the last row (R % 4 != 0) works on TMA zero-fill and stores nothing
+            const unsigned long long* mrow = maskbits && rin ? maskbits + ((long long)it.b * p.R + r) * NW : nullptr;
             uint64_t mb_next = mrow ? ldg_u64(mrow) : ~0ull;
             float m_run = -INFINITY, l_run = 0.0f;
             const long long off = (long long)it.b * p.sB + (long long)it.h * p.sH + (long long)r * p.sSlice + (long long)(it.q0 + row) * p.sPos;
@@ -308,7 +309,7 @@ sm100_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant_
                 warp_arrive(p_ready + g);
             }
             // ---- row epilogue: O = sigmoid(G) * O_r / l ; LSE = m + ln l -------------------------------
-            const bool inq = kAligned || it.q0 + row < N;  // the last query block may be partial
+            const bool inq = rin && (kAligned || it.q0 + row < N);  // the last query block may be partial
             uint4 gv[4];
             const uint4* gp = (const uint4*)(G + off);
 #pragma unroll
@@ -426,14 +427,14 @@ int sm100_sm_count() { return sm_count(); }
 // bias planes are read by TMA (16-byte row pitch in bf16).  N need not be a multiple of the 64 / 128-position tiles: TMA
 // zero-fills what lies beyond N, the packed mask hides keys >= N, stores of queries / keys >= N are predicated off.
 bool sm100_supported(const Problem& p, tri_dtype dt) {
-    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 8192 && p.R % 4 == 0 &&
+    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 8192 && p.R >= 1 &&
            (p.R == p.N || p.variant == TRI_STARTING);
 }
 
 // The forward alone has no cluster in it: its key loop is as long as N wants (long-sequence inference).  16384 keeps
 // every item count and TMA coordinate far inside 31 bits.
 bool sm100_fwd_supported(const Problem& p, tri_dtype dt) {
-    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 16384 && p.R % 4 == 0 &&
+    return dt == TRI_BF16 && p.d == 32 && p.N % 8 == 0 && p.N >= 128 && p.N <= 16384 && p.R >= 1 &&
            (p.R == p.N || p.variant == TRI_STARTING);
 }
 
@@ -470,7 +471,7 @@ tri_status sm100_fwd(const Problem& p, const void* Q, const void* K, const void*
     // the opt-in shared-memory size is a per-device function attribute: set it on every launch (cheap, thread-safe)
     auto kern = p.N % 128 == 0 ? sm100_fwd_kernel<true> : sm100_fwd_kernel<false>;
     TRI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdSmem::total));
-    const long long items = (long long)p.B * p.H * ((p.N + BQ - 1) / BQ) * (p.R / NG);
+    const long long items = (long long)p.B * p.H * ((p.N + BQ - 1) / BQ) * ((p.R + NG - 1) / NG);
     const int grid = (int)(items < sm_count() ? items : sm_count());
     {
         ProfScope ps("sm100_fwd_kernel", st);
