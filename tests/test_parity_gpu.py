@@ -649,3 +649,23 @@ def test_backward_beyond_n2048_runs_key_passes_on_the_tensor_core_kernels(tri, o
         oracle.bwd_start_general(x["dO"], x["Q"], x["K"], x["V"], x["G"], x["bias"], m))))
     errs = pu.assert_close(got, ref, pu.TOL["bf16"], what=f"key passes R={R} N={N}")
     print("key passes", R, N, {k: float(f"{v:.3g}") for k, v in errs.items()})
+
+
+@pytest.mark.parametrize("variant", [STARTING, ENDING])
+def test_autograd_front_end_matches_the_direct_calls(tri, variant):
+    """tri_attention (torch.autograd.Function over tri_attn_fwd / tri_attn_bwd): O and the gradients that loss.backward()
+    leaves in .grad are bitwise those of the direct calls (dBias after its cast to bf16)."""
+    import torch
+
+    cfg = tri_inputs.small_config(2, 128, 2, 32, "bf16", variant, 1.0, "random:5", seed=51)
+    x = tri_inputs.make_inputs(cfg)
+    _, direct = pu.run_gpu(x, "bf16", variant)
+    g = pu.gpu_inputs(x, "bf16")
+    leaves = {k: g[k].clone().requires_grad_(True) for k in ("Q", "K", "V", "G", "bias")}
+    O = tri.tri_attention(leaves["Q"], leaves["K"], leaves["V"], leaves["G"], leaves["bias"], g["mask"], variant)
+    (O.float() * g["dO"].float()).sum().backward()  # d loss / dO = dO exactly
+    torch.cuda.synchronize()
+    assert torch.equal(O.detach(), direct["O"])
+    for k, name in (("Q", "dQ"), ("K", "dK"), ("V", "dV"), ("G", "dG")):
+        assert torch.equal(leaves[k].grad, direct[name]), name
+    assert torch.equal(leaves["bias"].grad, direct["dBias"].to(torch.bfloat16))
