@@ -669,3 +669,12 @@ def test_autograd_front_end_matches_the_direct_calls(tri, variant):
     for k, name in (("Q", "dQ"), ("K", "dK"), ("V", "dV"), ("G", "dG")):
         assert torch.equal(leaves[k].grad, direct[name]), name
     assert torch.equal(leaves["bias"].grad, direct["dBias"].to(torch.bfloat16))
+
+
+def test_square_ending_node_beyond_n2048_sampled(tri, oracle):
+    """N = 2176 (34 key tiles: two key passes of 17), ending node, ragged tail mask, H = 1: the square entry points on the
+    tensor-core kernels; sampled rows and dBias lines against the oracle (strides of the ending-node layout in the fp32 dQ
+    carry between the passes)."""
+    cfg = tri_inputs.small_config(1, 2176, 1, 32, "bf16", ENDING, 1.5, "tail:53", seed=2176)
+    assert tri.uses_tensor_cores(1, 2176, 1, 32, ENDING, tri.BF16)
+    sampled_compare(oracle, cfg, n_rows=1, n_queries=1)
