@@ -477,9 +477,9 @@ def run_evosp(args, cfg):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if not dist.is_initialized():
-        if world > 1:
+        if "RANK" in os.environ and "MASTER_ADDR" in os.environ:  # torchrun (also with one rank): its rendezvous
             dist.init_process_group("nccl", device_id=dev)
-        else:
+        else:  # plain `python bench.py --sp`: a single-rank group of our own
             dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29517", rank=0, world_size=1, device_id=dev)
     tri.load()
     r0, n = evosp.shard_rows(cfg.N, world, rank)
