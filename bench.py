@@ -488,7 +488,7 @@ def run_evosp(args, cfg):
     g = {k: torch.from_numpy(x[k][:, r0:r0 + n].copy()).to(tdt).to(dev) for k in ("Q", "K", "V", "G", "dO")}
     bias_shard = torch.from_numpy(x["bias"][:, :, r0:r0 + n].copy()).to(tdt).to(dev)
     mask = None if x["mask"] is None else torch.from_numpy(x["mask"][:, r0:r0 + n].copy()).to(dev)
-    op = evosp.RowShardedTriAttention()
+    op = evosp.RowShardedTriAttention(peer_reduce=args.peer_reduce)
 
     def step():
         op.forward(g["Q"], g["K"], g["V"], g["G"], bias_shard, mask)
@@ -512,7 +512,8 @@ def run_evosp(args, cfg):
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": workload_name(cfg), "parallelism": f"sp{world}: {n} of {cfg.N} rows per rank, "
-                       "bias all-gather + dBias reduce-scatter inside the step"}}))
+                       "bias all-gather + dBias reduce-scatter inside the step"
+                       + (" (reduce-scatter: one kernel over peer memory)" if args.peer_reduce else " (NCCL)")}}))
     dist.destroy_process_group()
 
 
@@ -524,6 +525,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=sorted(tri_inputs.CONFIGS))
     ap.add_argument("--sp", action="store_true", help="EvoSP-3D row sharding of one batch (strong scaling)")
+    ap.add_argument("--peer-reduce", action="store_true",
+                    help="with --sp: dBias reduce-scatter by the peer-memory kernel (torch symmetric memory) instead of NCCL")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = tri_inputs.CONFIGS[args.workload]

@@ -161,6 +161,18 @@ TRI_API tri_status tri_attn_fwd_noalloc(const void* Q, const void* K, const void
                                 int B, int N, int H, int d, tri_variant variant, tri_dtype dtype,
                                 void* cuda_stream);
 
+/* EvoSP-3D, backward: reduce-scatter of the per-rank partial dBias as ONE kernel over peer memory.
+ * peer_dbias: HOST array of P DEVICE pointers, one per rank of the SP group in rank order, each to that rank's partial dBias
+ * [B,H,N,N] float32 (what tri_attn_rows_bwd wrote for the rank's rows); all must be loadable from the current device
+ * (peer access over NVLink / NVSwitch, e.g. torch symmetric memory, or buffers of the same device).  Writes
+ *     out_shard[b,h,l,k] = sum_{p = 0 .. P-1, ascending} peer_dbias[p][b,h, rank*(N/P) + l, k]     [B,H,N/P,N] float32
+ * i.e. this rank's N/P query lines of the total -- the sharding the bias was gathered from.  Fixed summation order:
+ * bitwise reproducible.  P <= 16, N % P == 0, N % 4 == 0, 16-byte aligned pointers, else TRI_ERR_UNSUPPORTED /
+ * TRI_ERR_INVALID_ARG.  The caller orders it after every peer's backward and keeps the peers from overwriting their
+ * buffers until all ranks have read them (paper_2506_20686_b200/evosp.py does both with the symmetric-memory barrier). */
+TRI_API tri_status tri_attn_dbias_reduce_scatter(const float* const* peer_dbias, int P, int rank, float* out_shard,
+                                         int B, int H, int N, void* cuda_stream);
+
 /* End-to-end step on HOST buffers: H2D(Q,K,V,G,bias,mask,dO) -> fwd -> bwd -> D2H(O,LSE,dQ,dK,dV,
  * dG,dBias).  `arena` is a caller-owned device buffer of tri_attn_step_host_arena_bytes() bytes. */
 TRI_API size_t tri_attn_step_host_arena_bytes(int B, int N, int H, int d, tri_variant variant, tri_dtype dtype);

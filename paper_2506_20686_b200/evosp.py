@@ -98,17 +98,49 @@ def rotate(x_shard: torch.Tensor, row_dim: int = 1, col_dim: int = 3, group=None
     return torch.cat(blocks, dim=col_dim).contiguous()
 
 
+class PeerReduceScatter:
+    """The dBias reduce-scatter as ONE kernel over peer memory (tri_attn_dbias_reduce_scatter) instead of an NCCL call:
+    every rank's partial dBias lives in a torch symmetric-memory buffer that its peers can load over NVLink / NVSwitch; each
+    rank sums its own N / P query lines out of all P buffers in rank order (fixed order: bitwise reproducible).
+
+        rs = PeerReduceScatter(B, H, N, group)       # collective: allocates and exchanges the buffers once
+        tri_attn_rows_bwd(..., out=(dQ, dK, dV, dG, rs.buffer))
+        dbias_shard = rs()                           # barrier, reduce kernel, barrier
+    """
+
+    def __init__(self, B: int, H: int, N: int, group=None, device=None):
+        import torch.distributed._symmetric_memory as symm_mem
+
+        group = dist.group.WORLD if group is None else group
+        device = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+        shard_rows(N, _world(group), dist.get_rank(group))  # N must divide evenly
+        self.shape = (B, H, N)
+        self.buffer = symm_mem.empty((B, H, N, N), dtype=torch.float32, device=device)
+        self.handle = symm_mem.rendezvous(self.buffer, group)
+
+    def __call__(self, out=None):
+        B, H, N = self.shape
+        h = self.handle
+        h.barrier()  # every rank's backward has written its buffer (stream-ordered on each rank)
+        out = binding.tri_attn_dbias_reduce_scatter(list(h.buffer_ptrs), h.rank, B, H, N, out=out, device=self.buffer.device)
+        h.barrier()  # nobody overwrites its buffer before every rank has read it
+        return out
+
+
 class RowShardedTriAttention:
     """Starting-node triangle attention on this rank's shard of the broadcast rows.
 
     forward(Q, K, V, G, bias_shard, mask) with Q,K,V,G [B,n,H,N,d] (rows r0..r0+n-1), bias_shard [B,H,n,N],
     mask [B,n,N] or None returns O [B,n,H,N,d] and LSE [B,n,H,N]; backward(dO) returns dQ, dK, dV, dG of
-    the local rows and dBias_shard [B,H,n,N] fp32 (already summed over the group).  For the ending-node
-    operator rotate() the operands first.  CUDA only."""
+    the local rows and dBias_shard [B,H,n,N] fp32 (already summed over the group; by NCCL reduce-scatter, or with
+    peer_reduce=True by the peer-memory kernel of PeerReduceScatter).  For the ending-node operator rotate() the
+    operands first.  CUDA only."""
 
-    def __init__(self, group=None):
+    def __init__(self, group=None, peer_reduce: bool = False):
         self.group = group
         self._saved = None
+        self._peer = peer_reduce  # dBias reduce-scatter by the peer-memory kernel instead of NCCL
+        self._rs = None
 
     def forward(self, Q, K, V, G, bias_shard, mask=None):
         if not Q.is_cuda:
@@ -125,5 +157,12 @@ class RowShardedTriAttention:
             raise binding.TriAttnError("backward() before forward()")
         Q, K, V, G, bias, mask, O, LSE = self._saved
         self._saved = None
-        dQ, dK, dV, dG, dBias = binding.tri_attn_rows_bwd(dO, Q, K, V, G, bias, mask, O, LSE)
-        return dQ, dK, dV, dG, scatter_dbias(dBias, self.group)
+        if not self._peer:
+            dQ, dK, dV, dG, dBias = binding.tri_attn_rows_bwd(dO, Q, K, V, G, bias, mask, O, LSE)
+            return dQ, dK, dV, dG, scatter_dbias(dBias, self.group)
+        B, _, H, N, _ = Q.shape
+        if self._rs is None or self._rs.shape != (B, H, N):
+            self._rs = PeerReduceScatter(B, H, N, self.group, Q.device)
+        grads = tuple(torch.empty_like(Q) for _ in range(4))
+        binding.tri_attn_rows_bwd(dO, Q, K, V, G, bias, mask, O, LSE, out=grads + (self._rs.buffer,))
+        return grads + (self._rs(),)

@@ -678,3 +678,43 @@ def test_square_ending_node_beyond_n2048_sampled(tri, oracle):
     cfg = tri_inputs.small_config(1, 2176, 1, 32, "bf16", ENDING, 1.5, "tail:53", seed=2176)
     assert tri.uses_tensor_cores(1, 2176, 1, 32, ENDING, tri.BF16)
     sampled_compare(oracle, cfg, n_rows=1, n_queries=1)
+
+
+def test_dbias_reduce_scatter_over_peer_buffers(tri):
+    """tri_attn_dbias_reduce_scatter: P = 3 partial dBias buffers (here all on one device; on a node they are the peers'
+    symmetric-memory buffers), every rank's shard = its N / P query lines summed over the buffers in rank order -- bitwise
+    the fp32 sum ((a + b) + c).  Then the same through PeerReduceScatter / RowShardedTriAttention(peer_reduce=True) on a
+    single-rank NCCL group with a torch symmetric-memory buffer: equal to the unsharded kernels."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2506_20686_b200 import evosp
+
+    B, H, N, P = 2, 3, 384, 3
+    torch.manual_seed(5)
+    parts = [torch.randn((B, H, N, N), dtype=torch.float32, device="cuda") for _ in range(P)]
+    want = (parts[0] + parts[1]) + parts[2]
+    n = N // P
+    for rank in range(P):
+        out = tri.tri_attn_dbias_reduce_scatter([t.data_ptr() for t in parts], rank, B, H, N)
+        torch.cuda.synchronize()
+        assert torch.equal(out, want[:, :, rank * n:(rank + 1) * n]), rank
+    with pytest.raises(tri.TriAttnError):
+        tri.tri_attn_dbias_reduce_scatter([t.data_ptr() for t in parts], 0, B, H, 400)  # N % P != 0
+
+    cfg = tri_inputs.small_config(1, 256, 2, 32, "bf16", STARTING, 1.0, "tail:20", seed=77)
+    x = tri_inputs.make_inputs(cfg)
+    _, full = pu.run_gpu(x, "bf16", STARTING)
+    g = pu.gpu_inputs(x, "bf16")
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29521", rank=0, world_size=1,
+                                device_id=torch.device("cuda", 0))
+    try:
+        op = evosp.RowShardedTriAttention(peer_reduce=True)
+        O, LSE = op.forward(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"])
+        outs = (O, LSE) + tuple(op.backward(g["dO"]))
+        torch.cuda.synchronize()
+        for k, v in zip(pu.OUT_NAMES, outs):
+            assert torch.equal(v, full[k]), k
+    finally:
+        dist.destroy_process_group()
