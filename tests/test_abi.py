@@ -113,3 +113,28 @@ def test_binding_refuses_cpu_tensors(lib):
     x = torch.zeros(1, 4, 1, 4, 32)
     with pytest.raises(TriAttnError):
         tri_attn_fwd(x, x, x, x, torch.zeros(1, 1, 4, 4))
+
+
+def test_rows_and_peer_entry_points_validate_before_any_launch(lib):
+    """The newer entry points (rows, no-alloc, peer reduce-scatter) reject bad arguments without a GPU and without a launch."""
+    n0 = lib.tri_attn_launch_count()
+    p = ctypes.c_void_p(4096)
+    # rows: unsupported dtype / head dim / N not a multiple of 8 -> workspace 0 and TRI_ERR_UNSUPPORTED; bad R -> invalid
+    assert lib.tri_attn_rows_fwd_workspace_bytes(1, 8, 128, 2, 32, 0) == 0
+    assert lib.tri_attn_rows_fwd_workspace_bytes(1, 8, 132, 2, 32, 1) == 0
+    assert lib.tri_attn_rows_fwd_workspace_bytes(1, 1, 128, 2, 32, 1) > 0          # any R >= 1
+    assert lib.tri_attn_rows_bwd_workspace_bytes(1, 8, 16384, 1, 32, 1) == 0       # backward stops at N = 8192 ...
+    assert lib.tri_attn_rows_fwd_workspace_bytes(1, 8, 16384, 1, 32, 1) > 0        # ... the forward at 16384
+    assert lib.tri_attn_rows_fwd(p, p, p, p, p, None, p, p, 1, 0, 128, 2, 32, 1, p, 1 << 20, None) == 1
+    assert lib.tri_attn_rows_fwd(p, p, p, p, p, None, p, p, 1, 8, 128, 2, 64, 1, p, 1 << 20, None) == 2
+    assert lib.tri_attn_rows_bwd(*([p] * 6), None, *([p] * 7), 1, 8, 128, 2, 32, 1, None, 0, None) == 3
+    # peer reduce-scatter
+    arr = (ctypes.c_void_p * 3)(4096, 8192, 12288)
+    ptrs = ctypes.cast(arr, ctypes.c_void_p)
+    assert lib.tri_attn_dbias_reduce_scatter(None, 3, 0, p, 1, 2, 384, None) == 1
+    assert lib.tri_attn_dbias_reduce_scatter(ptrs, 3, 3, p, 1, 2, 384, None) == 1      # rank outside the group
+    assert lib.tri_attn_dbias_reduce_scatter(ptrs, 3, 0, p, 1, 2, 400, None) == 2      # N % P != 0
+    assert lib.tri_attn_dbias_reduce_scatter(ptrs, 17, 0, p, 1, 2, 17 * 16, None) == 2  # more than 16 peers
+    arr_bad = (ctypes.c_void_p * 3)(4096, 8200, 12288)
+    assert lib.tri_attn_dbias_reduce_scatter(ctypes.cast(arr_bad, ctypes.c_void_p), 3, 0, p, 1, 2, 384, None) == 1  # misaligned peer
+    assert lib.tri_attn_launch_count() == n0
