@@ -1,7 +1,7 @@
 // fp32 CUDA-core kernels for triangle attention (any N, d in {16,32,64}, f32 or bf16 storage).
 //
 // This is the path for dtype f32 (the 1e-4 tolerance excludes TF32 tensor cores, A14) and
-// for bf16 shapes the tcgen05 kernels do not cover (N % 128 != 0 or d != 32).  Same structure as
+// for bf16 shapes the tcgen05 kernels do not cover (N % 8 != 0, N < 128 or d != 32).  Same structure as
 // the paper's kernels: flash-style online-softmax forward (Listing 1), backward =
 // preprocess D + key-stationary dK/dV + query-stationary dQ;
 // dBias is a third, tile-stationary kernel that sums dS over the broadcast axis in ascending order

@@ -2,13 +2,15 @@
 // (Listing 2 stage 2; Table I).  The paper adds its dS tiles into dBias with tl.atomic_add
 // (P:L488); here the reduction over the broadcast rows is deterministic and on-chip:
 //
-//   * tile-stationary: a CTA owns the dBias tiles (128 queries x up to 3 x 64 keys) of one (b, h) in REGISTERS and
+//   * tile-stationary: a CTA owns the dBias tiles (128 queries x up to 2 x 64 keys) of one (b, h) in REGISTERS and
 //     streams over the broadcast rows r in ascending order (level 1 of the dBias reduction; level 2, only when the
 //     row axis is split over G CTAs to fill the SMs, is sm100_dbias_reduce_kernel);
 //   * the CTAs that own the key tiles of one 128-query block form a thread-block CLUSTER; each accumulates its
 //     partial dQ_r = sum over its keys of dS K in TMEM, and the partials of a row are added in rank order through
 //     distributed shared memory (rank c receives the running sum of ranks < c, adds its own, passes it on; the last
 //     rank scales and stores dQ).  No floating-point atomics anywhere; every output is bitwise reproducible.
+//     A cluster has at most 16 ranks = 2048 keys; N > 2048 runs ceil(N / 2048) launches over slices of the key axis
+//     (DqdbPass, template flag kPasses): dBias columns are disjoint per slice, dQ is carried as an fp32 sum in global memory.
 //
 // Persistent, warp-specialised CTA of 512 threads:
 //   warps 0-7    two compute groups (128 threads = 128 query rows = 128 TMEM lanes); group g owns key tile g of the CTA,
