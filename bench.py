@@ -419,6 +419,15 @@ def run_ours(args, cfg):
         if fl is not None:
             roof["mufu_co_roofline"] = {"exp_floor_ms": fl, "frac": fl / (dms / dn),
                                         "note": "one ex2 per logit and pass at 148 SM x 16/clk"}
+        # second co-bound: HBM.  Algorithmic bytes of the whole step = 15 U (fwd: Q,K,V,G in, O out;
+        # bwd: Q,K,V,G,O,dO in, dQ,dK,dV,dG out) + bias x 2, LSE x 2, dBias, mask; of the dominant kernel = 5 U.
+        es = 2 if cfg.dtype == "bf16" else 4
+        U = B * N * H * N * d * es
+        step_bytes = 15 * U + 2 * B * H * N * N * es + 2 * B * N * H * N * 4 + B * H * N * N * 4 + (B * N * N if host["mask"] is not None else 0)
+        roof["hbm_co_roofline"] = {"step_algorithmic_gb": step_bytes / 1e9, "step_achieved_gbs": step_bytes / (ms_step * 1e-3) / 1e9,
+                                   "kernel_algorithmic_gb": 5 * U / 1e9, "kernel_achieved_gbs": 5 * U / (dms / dn * 1e-3) / 1e9,
+                                   "peak_gbs": peaks["hbm_gbs"], "step_frac": step_bytes / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                   "hbm_floor_ms": step_bytes / peaks["hbm_gbs"] / 1e6}
     else:
         U = B * N * H * N * d * (2 if cfg.dtype == "bf16" else 4)
         bytes_ = 4 * U + B * N * H * N * 4  # preprocess: read dO,O,G, write dG + D
