@@ -267,12 +267,19 @@ class DeviceProblem:
                             tri.bwd_workspace_bytes(B, N, H, d, cfg.variant, self.code))
         self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=dev)
 
-    def step(self):
+    def fwd(self):
         g, cfg, tri = self.g, self.cfg, self.tri
         tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], cfg.variant, O=self.O, LSE=self.LSE,
                          workspace=self.ws)
+
+    def bwd(self):
+        g, cfg, tri = self.g, self.cfg, self.tri
         tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], self.O, self.LSE, cfg.variant,
                          out=self.grads, workspace=self.ws)
+
+    def step(self):
+        self.fwd()
+        self.bwd()
 
 
 def time_steps(prob, steps, warmup, barrier):
@@ -340,6 +347,22 @@ def run_ours(args, cfg):
     ms_step = max_over_ranks(ms_step, dev, world)
     flop_all = model_flop(cfg) * world
     value = aggregate_value(cfg, world, ms_step)
+
+    # ---- forward and backward on their own (outside the timed region; SURVEY Sec. 8(d) bench protocol)
+    def phase_ms(fn, n):
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    n_ph = max(3, min(args.steps, 20))
+    phases = {"fwd_ms": phase_ms(prob.fwd, n_ph), "bwd_ms": phase_ms(prob.bwd, n_ph), "iterations": n_ph}
+    phases["fwd_tflops"] = 4.0 / 14.0 * model_flop(cfg) / (phases["fwd_ms"] * 1e-3) / 1e12
+    phases["bwd_tflops"] = 10.0 / 14.0 * model_flop(cfg) / (phases["bwd_ms"] * 1e-3) / 1e12
 
     # ---- per-kernel times: a second, separately profiled loop (events around every launch inside the library)
     prof_steps = max(3, min(args.steps, 10))
@@ -459,7 +482,7 @@ def run_ours(args, cfg):
                                              "sm100_dkdv_kernel(side) beside sm100_dqdb_kernel on the SMs its clusters leave empty, "
                                              "sm100_dbias_reduce_kernel beside the rest of sm100_dkdv_kernel -- so their event brackets include "
                                              "the time they share the GPU; `share` is taken over the caller-stream kernels only",
-        "roofline": roof, "also": also, "cpu_baseline": cpu,
+        "phases": phases, "roofline": roof, "also": also, "cpu_baseline": cpu,
         "e2e": {"value": flop_all / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,
