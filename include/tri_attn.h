@@ -170,6 +170,11 @@ TRI_API tri_status tri_attn_fwd_noalloc(const void* Q, const void* K, const void
  * bitwise reproducible.  P <= 16, N % P == 0, N % 4 == 0, 16-byte aligned pointers, else TRI_ERR_UNSUPPORTED /
  * TRI_ERR_INVALID_ARG.  The caller orders it after every peer's backward and keeps the peers from overwriting their
  * buffers until all ranks have read them (paper_2506_20686_b200/evosp.py does both with the symmetric-memory barrier). */
+/* EvoSP-3D, forward: all-gather of the bias by pulling over peer memory.  peer_shards: HOST array of P DEVICE
+ * pointers in rank order, each to that rank's shard [B,H,N/P,N] (`dtype`) of query lines; writes the full out_bias [B,H,N,N]
+ * on this device.  Same peer-access, alignment (16 bytes; N * sizeof(elem) % 16 == 0), P <= 16 and ordering rules as below. */
+TRI_API tri_status tri_attn_bias_all_gather(const void* const* peer_shards, int P, void* out_bias, int B, int H, int N,
+                                    tri_dtype dtype, void* cuda_stream);
 TRI_API tri_status tri_attn_dbias_reduce_scatter(const float* const* peer_dbias, int P, int rank, float* out_shard,
                                          int B, int H, int N, void* cuda_stream);
 

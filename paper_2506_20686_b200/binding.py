@@ -33,6 +33,7 @@ SIGNATURES = {
     "tri_attn_noalloc_scratch_bytes": (_sz, []),
     "tri_attn_fwd_noalloc": (_i, [_vp] * 8 + [_i] * 6 + [_vp]),
     "tri_attn_dbias_reduce_scatter": (_i, [_vp, _i, _i, _vp, _i, _i, _i, _vp]),
+    "tri_attn_bias_all_gather": (_i, [_vp, _i, _vp, _i, _i, _i, _i, _vp]),
     "tri_attn_step_host_arena_bytes": (_sz, [_i] * 6),
     "tri_attn_step_host": (_i, [_vp] * 14 + [_i] * 6 + [_vp, _sz, _vp]),
     "tri_attn_uses_tensor_cores": (_i, [_i] * 6),
@@ -289,6 +290,23 @@ def tri_attn_fwd_noalloc(Q, K, V, G, bias, mask, variant, O, LSE):
         _check(lib.tri_attn_fwd_noalloc(_ptr(Q), _ptr(K), _ptr(V), _ptr(G), _ptr(bias), _ptr(mask), _ptr(O), _ptr(LSE),
                                         B, N, H, d, variant, _dtype_code(Q), stream))
     return O, LSE
+
+
+def tri_attn_bias_all_gather(peer_ptrs, B, H, N, dtype, out=None, device=None):
+    """bias [B,H,N,N] assembled from the P ranks' shards [B,H,N/P,N] (device pointers in rank order), by pulling."""
+    lib = load()
+    P = len(peer_ptrs)
+    if P == 0 or N % P:
+        raise TriAttnError(f"N={N} is not a multiple of the group size {P}")
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+    if out is None:
+        out = torch.empty((B, H, N, N), dtype=dtype, device=dev)
+    _chk(out, (B, H, N, N), dtype, "out", dev)
+    arr = (ctypes.c_void_p * P)(*[int(p) for p in peer_ptrs])
+    with torch.cuda.device(dev):
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(lib.tri_attn_bias_all_gather(ctypes.cast(arr, ctypes.c_void_p), P, _ptr(out), B, H, N, _dtype_code(out), stream))
+    return out
 
 
 def tri_attn_dbias_reduce_scatter(peer_ptrs, rank, B, H, N, out=None, device=None):

@@ -127,27 +127,63 @@ class PeerReduceScatter:
         return out
 
 
+class PeerAllGather:
+    """The bias all-gather as a pull over peer memory (tri_attn_bias_all_gather): every rank puts its shard [B,H,n,N] into a
+    torch symmetric-memory buffer and copies the lines of all shards into its own full bias with one kernel.
+
+        ag = PeerAllGather(B, H, N, dtype, group)     # collective: allocates and exchanges the buffers once
+        bias = ag(bias_shard)                          # local copy into the buffer, barrier, pull kernel, barrier
+    """
+
+    def __init__(self, B: int, H: int, N: int, dtype, group=None, device=None):
+        import torch.distributed._symmetric_memory as symm_mem
+
+        group = dist.group.WORLD if group is None else group
+        device = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+        _, n = shard_rows(N, _world(group), dist.get_rank(group))
+        self.shape = (B, H, N)
+        self.buffer = symm_mem.empty((B, H, n, N), dtype=dtype, device=device)
+        self.handle = symm_mem.rendezvous(self.buffer, group)
+
+    def __call__(self, bias_shard, out=None):
+        B, H, N = self.shape
+        h = self.handle
+        self.buffer.copy_(bias_shard)
+        h.barrier()  # every rank's shard is in its buffer
+        out = binding.tri_attn_bias_all_gather(list(h.buffer_ptrs), B, H, N, self.buffer.dtype, out=out, device=self.buffer.device)
+        h.barrier()  # nobody refills its buffer before every rank has read it
+        return out
+
+
 class RowShardedTriAttention:
     """Starting-node triangle attention on this rank's shard of the broadcast rows.
 
     forward(Q, K, V, G, bias_shard, mask) with Q,K,V,G [B,n,H,N,d] (rows r0..r0+n-1), bias_shard [B,H,n,N],
     mask [B,n,N] or None returns O [B,n,H,N,d] and LSE [B,n,H,N]; backward(dO) returns dQ, dK, dV, dG of
     the local rows and dBias_shard [B,H,n,N] fp32 (already summed over the group; by NCCL reduce-scatter, or with
-    peer_reduce=True by the peer-memory kernel of PeerReduceScatter).  For the ending-node operator rotate() the
+    peer_reduce=True the bias all-gather and the dBias reduce-scatter both run as our kernels over peer memory:
+    PeerAllGather, PeerReduceScatter).  For the ending-node operator rotate() the
     operands first.  CUDA only."""
 
     def __init__(self, group=None, peer_reduce: bool = False):
         self.group = group
         self._saved = None
-        self._peer = peer_reduce  # dBias reduce-scatter by the peer-memory kernel instead of NCCL
+        self._peer = peer_reduce  # both exchanges by the peer-memory kernels (symmetric memory) instead of NCCL
         self._rs = None
+        self._ag = None
 
     def forward(self, Q, K, V, G, bias_shard, mask=None):
         if not Q.is_cuda:
             raise binding.TriAttnError("RowShardedTriAttention needs CUDA tensors (there is no CPU path)")
-        work, finish = gather_bias(bias_shard, self.group, async_op=True)
-        work.wait()  # stream-ordered for NCCL: the kernels below are enqueued behind the all-gather
-        bias = finish().contiguous()
+        if self._peer:
+            B, H, n, N = bias_shard.shape
+            if self._ag is None or self._ag.shape != (B, H, N) or self._ag.buffer.dtype != bias_shard.dtype:
+                self._ag = PeerAllGather(B, H, N, bias_shard.dtype, self.group, Q.device)
+            bias = self._ag(bias_shard)
+        else:
+            work, finish = gather_bias(bias_shard, self.group, async_op=True)
+            work.wait()  # stream-ordered for NCCL: the kernels below are enqueued behind the all-gather
+            bias = finish().contiguous()
         O, LSE = binding.tri_attn_rows_fwd(Q, K, V, G, bias, mask)
         self._saved = (Q, K, V, G, bias, mask, O, LSE)
         return O, LSE

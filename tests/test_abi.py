@@ -135,6 +135,9 @@ def test_rows_and_peer_entry_points_validate_before_any_launch(lib):
     assert lib.tri_attn_dbias_reduce_scatter(ptrs, 3, 3, p, 1, 2, 384, None) == 1      # rank outside the group
     assert lib.tri_attn_dbias_reduce_scatter(ptrs, 3, 0, p, 1, 2, 400, None) == 2      # N % P != 0
     assert lib.tri_attn_dbias_reduce_scatter(ptrs, 17, 0, p, 1, 2, 17 * 16, None) == 2  # more than 16 peers
+    assert lib.tri_attn_bias_all_gather(None, 3, p, 1, 2, 384, 1, None) == 1
+    assert lib.tri_attn_bias_all_gather(ptrs, 3, p, 1, 2, 400, 1, None) == 2           # N % P != 0
+    assert lib.tri_attn_bias_all_gather(ptrs, 3, p, 1, 2, 384, 7, None) == 1           # bad dtype
     arr_bad = (ctypes.c_void_p * 3)(4096, 8200, 12288)
     assert lib.tri_attn_dbias_reduce_scatter(ctypes.cast(arr_bad, ctypes.c_void_p), 3, 0, p, 1, 2, 384, None) == 1  # misaligned peer
     assert lib.tri_attn_launch_count() == n0

@@ -701,6 +701,12 @@ def test_dbias_reduce_scatter_over_peer_buffers(tri):
         assert torch.equal(out, want[:, :, rank * n:(rank + 1) * n]), rank
     with pytest.raises(tri.TriAttnError):
         tri.tri_attn_dbias_reduce_scatter([t.data_ptr() for t in parts], 0, B, H, 400)  # N % P != 0
+    # the pull all-gather: the full bias from three shards of query lines
+    full_bias = torch.randn((B, H, N, N), device="cuda").to(torch.bfloat16)
+    shards = [full_bias[:, :, r * n:(r + 1) * n].contiguous() for r in range(P)]
+    got_bias = tri.tri_attn_bias_all_gather([t.data_ptr() for t in shards], B, H, N, torch.bfloat16)
+    torch.cuda.synchronize()
+    assert torch.equal(got_bias, full_bias)
 
     cfg = tri_inputs.small_config(1, 256, 2, 32, "bf16", STARTING, 1.0, "tail:20", seed=77)
     x = tri_inputs.make_inputs(cfg)
