@@ -41,6 +41,9 @@
  *     least *_workspace_bytes() bytes, contents undefined on entry and exit).  workspace_bytes is
  *     O(B*H*N^2*d) (the backward keeps one dA = dO (.) sigmoid(G) tensor there); nothing of size
  *     B*H*N^3 exists anywhere.
+ *   - Thread safety: entry points may be called from several host threads (on the same or different devices and
+ *     streams); enqueues that share a device's side streams take turns inside the library.  The exceptions are the
+ *     profiling calls (one thread) and tri_attn_fwd_noalloc (overlapping calls race on its built-in scratch).
  *   - tri_attn_fwd / tri_attn_bwd / tri_attn_rows_* enqueue stream work only (kernels and the event fork / join of the
  *     side streams), so a step can be captured into a CUDA graph on `cuda_stream` and replayed (tested; make one eager
  *     call first so that the library's streams, events and tensor maps exist before the capture).

@@ -108,6 +108,7 @@ struct SideStream {
     cudaStream_t hi = nullptr;                     // high-priority stream of the dBias plane reduction
     cudaEvent_t stage2 = nullptr, join2 = nullptr; // stage 2 done -> reduction (beside the rest of stage 1) -> joined
     bool ready = false;
+    std::mutex enqueue;  // held while one call enqueues: the stream and the events are shared by all callers on the device
 };
 std::mutex g_side_mu;
 SideStream g_side[64];
@@ -153,6 +154,10 @@ tri_status sm100_bwd(const Problem& p, const void* dO, const void* Q, const void
     // work on `st`).  It carries (1) the bias / mask preparation, which is independent of the HBM-bound pre-process kernel,
     // (2) a slice of stage 1 beside stage 2, (3) the dBias plane reduction beside the rest of stage 1.
     SideStream* side = side_stream();
+    // Host threads that call on one device share the side streams and their events: their enqueues take turns (a stream wait
+    // captures the event's state when it is enqueued, so a later re-record by another caller does not disturb it).
+    std::unique_lock<std::mutex> enqueue_lock;
+    if (side) enqueue_lock = std::unique_lock<std::mutex>(side->enqueue);
     cudaStream_t sp = side ? side->stream : st;  // where the preparation kernels go
     if (side) {
         TRI_CUDA_CHECK(cudaEventRecord(side->fork0, st));

@@ -724,3 +724,44 @@ def test_dbias_reduce_scatter_over_peer_buffers(tri):
             assert torch.equal(v, full[k]), k
     finally:
         dist.destroy_process_group()
+
+
+def test_two_host_threads_on_one_device(tri):
+    """Two host threads, each on its own CUDA stream, run forward + backward of different problems at the same time (ctypes
+    drops the GIL inside the calls, so the enqueues really interleave; the library's side streams and events are shared per
+    device).  Each thread's results must be bitwise those of a serial run."""
+    import threading
+
+    import torch
+
+    cfgs = [tri_inputs.small_config(2, 256, 2, 32, "bf16", STARTING, 1.0, "random:7", seed=901),
+            tri_inputs.small_config(1, 384, 3, 32, "bf16", ENDING, 1.0, "tail:9", seed=902)]
+    xs = [tri_inputs.make_inputs(c) for c in cfgs]
+    serial = [pu.run_gpu(x, "bf16", c.variant)[1] for x, c in zip(xs, cfgs)]
+    gs = [pu.gpu_inputs(x, "bf16") for x in xs]
+    torch.cuda.synchronize()
+    results, errors = [None, None], []
+
+    def work(i):
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                g, c = gs[i], cfgs[i]
+                for _ in range(10):
+                    O, LSE = tri.tri_attn_fwd(g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], c.variant)
+                    outs = tri.tri_attn_bwd(g["dO"], g["Q"], g["K"], g["V"], g["G"], g["bias"], g["mask"], O, LSE, c.variant)
+                s.synchronize()
+                results[i] = (O, LSE) + tuple(outs)
+        except Exception as e:  # noqa: BLE001
+            errors.append(e)
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for i in range(2):
+        for k, v in zip(pu.OUT_NAMES, results[i]):
+            assert torch.equal(v.view(torch.uint8), serial[i][k].view(torch.uint8)), (i, k)
