@@ -380,3 +380,33 @@ def test_general_shape_core_is_consistent_with_square(oracle):
     np.testing.assert_array_equal(gq[0], dQ[:, :, :, qs])
     np.testing.assert_array_equal(gq[3], dG[:, :, :, qs])
     np.testing.assert_array_equal(gq[4], dB[:, :, qs])
+
+
+def test_general_shape_dbias_is_additive_over_row_partitions_and_rows_may_exceed_n(oracle):
+    """What the row-chunked host pipeline, the EvoSP row shards and the R != N entry points rely on: with the bias plane
+    fixed, the rows are independent problems, so dBias of a row set is the sum of the dBias of any partition of it (here
+    against the square problem's dBias), a single row (R = 1) is a legal problem, and R may exceed N (rows of two unrelated
+    draws stacked: every per-row output equals that of the problem the row came from)."""
+    B, N, H, d = 1, 6, 2, 4
+    p = rand_problem(B, N, H, d, seed=61, mask_p=0.25)
+    q = rand_problem(B, N, H, d, seed=62, mask_p=0.25)
+    a = (p["Q"], p["K"], p["V"], p["G"], p["bias"], p["mask"])
+    dB_all = oracle.bwd(p["dO"], *a, S)[4]
+    parts = ([0], [1, 2, 3], [4, 5])
+    acc = np.zeros_like(dB_all)
+    for rows in parts:
+        acc += oracle.bwd_start_general(p["dO"][:, rows], p["Q"][:, rows], p["K"][:, rows], p["V"][:, rows], p["G"][:, rows],
+                                        p["bias"], p["mask"][:, rows])[4]
+    np.testing.assert_allclose(acc, dB_all, rtol=1e-13, atol=1e-14)
+    # R = 2 N rows: p's rows followed by q's rows, all under p's bias
+    cat = {k: np.concatenate([p[k], q[k]], axis=1) for k in ("Q", "K", "V", "G", "dO", "mask")}
+    O2, L2 = oracle.fwd_start_general(cat["Q"], cat["K"], cat["V"], cat["G"], p["bias"], cat["mask"])
+    g2 = oracle.bwd_start_general(cat["dO"], cat["Q"], cat["K"], cat["V"], cat["G"], p["bias"], cat["mask"])
+    Op, Lp = oracle.fwd(*a, S)
+    Oq, Lq = oracle.fwd_start_general(q["Q"], q["K"], q["V"], q["G"], p["bias"], q["mask"])
+    np.testing.assert_array_equal(O2[:, :N], Op)
+    np.testing.assert_array_equal(O2[:, N:], Oq)
+    np.testing.assert_array_equal(L2[:, :N], Lp)
+    gq = oracle.bwd_start_general(q["dO"], q["Q"], q["K"], q["V"], q["G"], p["bias"], q["mask"])
+    np.testing.assert_array_equal(g2[0][:, N:], gq[0])
+    np.testing.assert_allclose(g2[4], dB_all + gq[4], rtol=1e-13, atol=1e-14)
